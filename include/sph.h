@@ -1,0 +1,208 @@
+/*
+ * sph.h -- C ABI of libsph_b200: the per-time-step DFSPH particle pipeline of
+ * arxiv 2403.11156 ("Journey into SPH Simulation") as hand-written CUDA for sm_100a.
+ *
+ * Citations are /root/reference/PAPER.md line numbers (section / equation named) and the
+ * readings Rn of DESIGN.md (the paper prints no DFSPH equations, no kernel function and no
+ * neighbour-search description; every gap is an explicit reading there).
+ *
+ * Conventions
+ *   - every function returns SPH_OK (0) or a negative SphError; nothing throws across the ABI;
+ *     sph_last_error() gives the text of the last failure of that simulation (or of create).
+ *   - the library NEVER allocates or frees device memory: the caller (PyTorch tensors in the
+ *     Python binding) owns the inputs and one workspace of sph_workspace_bytes() bytes that
+ *     must stay alive and untouched until sph_destroy().  It creates one helper stream (used
+ *     only to capture CUDA-graph loop bodies, never to run work) and a few KB of pinned host
+ *     memory.
+ *   - all work is enqueued asynchronously on the cudaStream_t given to sph_create(); the only
+ *     calls that synchronise that stream are sph_read_stats(), host-buffer copies of
+ *     sph_read_state()/sph_write_state(), sph_create() itself (it computes the Akinci
+ *     volumes) and the step calls when SphParams.use_cuda_graph == 0 (debug mode: the
+ *     solver loops are then driven from the host).
+ *   - "device" pointers are CUDA device pointers on `cuda_device`; "host" pointers are
+ *     ordinary (preferably pinned) host memory.
+ *   - particles are handed over and read back in the caller's ORIGINAL id order; internally
+ *     the store is kept sorted by grid cell (SoA float4, fp32) and re-sorted every step.
+ *   - device-side conditions (particles clamped at the grid edge, neighbour-list overflow,
+ *     NaN, max-iterations reached) are counters in SphStats, not return codes.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_ABI_VERSION 1
+
+typedef enum SphError {
+    SPH_OK = 0,
+    SPH_EINVAL = -1,  /* bad argument / inconsistent parameters */
+    SPH_ENOMEM = -2,  /* workspace too small */
+    SPH_ECUDA = -3,   /* a CUDA runtime call failed (text in sph_last_error) */
+    SPH_EDOMAIN = -4, /* grid would exceed 2^31 cells or domain is empty */
+    SPH_ESTATE = -5   /* call not valid in this state (e.g. read of a field not yet computed) */
+} SphError;
+
+/* Problem statement ("domain boundary, simulation method, particle radius,
+ * support radius, density, viscosity, initial position, velocity"; PAPER.md:140 k, gamma;
+ * PAPER.md:170 "max error").  Plain C struct, passed by pointer, copied by sph_create. */
+typedef struct SphParams {
+    float particle_radius;     /* r */
+    float support_radius;      /* h, support radius of W (= 4r) */
+    float rest_density;        /* rho0 */
+    float particle_mass;       /* 0 => rho0 (2r)^3                    reading R3 */
+    float dt;                  /* fixed time step                     reading R19 */
+    float gravity[3];
+    float domain_min[3];       /* grid origin and extent; particles outside are clamped into */
+    float domain_max[3];       /*   the edge cells and counted in SphStats.oob_count (R11)   */
+    float tank_min[3];         /* AABB used only by the rigid-body wall-contact stand-in (R18) */
+    float tank_max[3];
+    int   viscosity_mode;      /* 0 none, 1 explicit Eq. 15, 2 implicit Eq. 16-19 (CG) */
+    float kinematic_viscosity; /* nu = mu / rho0 */
+    float cg_rel_tol;          /* |r|_2 <= tol |b|_2                  reading R23 */
+    int   cg_max_iter;
+    float eta_density;         /* mean(rho* - rho0)/rho0 threshold    reading R6 */
+    int   min_iter_density, max_iter_density;
+    float eta_divergence;      /* dt mean(Drho/Dt)/rho0 threshold     reading R6 */
+    int   min_iter_divergence, max_iter_divergence;
+    int   enable_divergence_solve;
+    int   force_iterations;    /* 1: run exactly min_iter_* iterations, ignore the errors */
+    float wcsph_stiffness;     /* k */
+    float wcsph_exponent;      /* gamma */
+    int   max_fluid_neighbors;    /* capacity of the per-particle fluid neighbour list, 0 => 64;
+                                     rounded up to a multiple of 4.  Overflow is counted in
+                                     SphStats.overflow_count and the step's results are invalid */
+    int   max_boundary_neighbors; /* same for boundary neighbours, 0 => 64 */
+    int   use_cuda_graph;      /* 1: one CUDA graph per step with device-side WHILE loops (default
+                                  path); 0: plain launches, loop predicates read by the host */
+    int   use_neighbor_list;   /* 1: solver passes gather through the per-step neighbour list
+                                  (default); 0: every pass re-walks the 27 cells */
+} SphParams;
+
+/* Rigid body = contiguous range of boundary samples (Akinci [3]).  Dynamics are
+ * a minimal stand-in for the external engine the paper delegates to (R18). */
+typedef struct SphRigidBody {
+    int   first_particle, n_particles; /* range in the boundary arrays (original order) */
+    int   dynamic;                     /* 0: static (walls, obstacles) */
+    float mass;
+    float inertia_body[3];             /* principal moments, body frame */
+    float com[3];
+    float quat[4];                     /* w, x, y, z */
+    float lin_vel[3];
+    float ang_vel[3];
+    float contact_radius;              /* wall-contact sphere radius of the stand-in */
+} SphRigidBody;
+
+/* Inputs of sph_create; all DEVICE pointers, owned by the caller, read during sph_create only
+ * (copied into the workspace), except `workspace` which the simulation lives in. */
+typedef struct SphBuffers {
+    const float *fluid_pos;      /* [n_fluid * 3] xyz, original id order */
+    const float *fluid_vel;      /* [n_fluid * 3] */
+    const float *boundary_pos;   /* [n_boundary * 3] world coordinates at t = 0 (may be NULL if 0) */
+    const int   *boundary_body;  /* [n_boundary] index into bodies[] */
+    void        *workspace;      /* >= sph_workspace_bytes(...), 256-byte aligned */
+    size_t       workspace_bytes;
+} SphBuffers;
+
+typedef struct SphStats {
+    long long steps_done;        /* steps since create */
+    long long total_it_v;        /* summed over steps_done (mean iterations = total / steps) */
+    long long total_it_d;
+    long long total_cg_iters;
+    int   it_v, it_d, cg_iters;  /* last step */
+    float err_v, err_rho;        /* last step: errors measured in the last P-pass (R14) */
+    float cg_residual;           /* |r|/|b| at exit */
+    int   oob_count;             /* fluid particles clamped into edge cells in the last grid build */
+    int   overflow_count;        /* particles whose neighbour list overflowed (last step) */
+    int   nan_count;             /* fluid particles with a non-finite position or velocity after the step */
+    int   max_iter_hit;          /* bit 0: divergence, bit 1: density, bit 2: CG reached max iterations */
+    float v_max;                 /* max |v| after the last step (CFL monitor) */
+    int   max_fluid_neighbors;   /* largest fluid / boundary neighbour count seen in the last list build */
+    int   max_boundary_neighbors;
+    float mean_fluid_neighbors;
+} SphStats;
+
+/* Fields of sph_read_state / sph_write_state.  Per-particle fields are in ORIGINAL id order. */
+typedef enum SphField {
+    SPH_FIELD_POS = 0,             /* float [n_fluid*3]                                  rw */
+    SPH_FIELD_VEL = 1,             /* float [n_fluid*3]                                  rw */
+    SPH_FIELD_DENSITY = 2,         /* float [n_fluid]   rho_i of the last density pass (Eq. 4 + 12) */
+    SPH_FIELD_ALPHA = 3,           /* float [n_fluid]   DFSPH factor (R5) */
+    SPH_FIELD_KAPPA_OVER_RHO = 4,  /* float [n_fluid]   kappa_i / rho_i of the last P-pass (WCSPH: p_i / rho~_i^2) */
+    SPH_FIELD_CELL_START = 5,      /* int   [n_cells+1] fluid grid, linear x-fastest cell order (R11) */
+    SPH_FIELD_CELL_OF_PARTICLE = 6,/* int   [n_fluid]   linear cell key of every fluid particle */
+    SPH_FIELD_SORTED_ID = 7,       /* int   [n_fluid]   original id of the particle in sorted slot s */
+    SPH_FIELD_NEIGHBOR_COUNT = 8,  /* int   [n_fluid*2] (#fluid, #boundary) neighbours */
+    SPH_FIELD_FLUID_NEIGHBORS = 9, /* int   [n_fluid*Kf] original ids of fluid neighbours, -1 padded (Kf = fluid list capacity) */
+    SPH_FIELD_BOUNDARY_NEIGHBORS = 10, /* int [n_fluid*Kb] original boundary ids, -1 padded */
+    SPH_FIELD_BOUNDARY_POS = 11,   /* float [n_boundary*3] current world positions           rw */
+    SPH_FIELD_BOUNDARY_VEL = 12,   /* float [n_boundary*3]                                   rw */
+    SPH_FIELD_BOUNDARY_PSI = 13,   /* float [n_boundary]   Akinci Psi_k (Eq. 11) */
+    SPH_FIELD_BOUNDARY_FORCE = 14, /* float [n_boundary*3] Eq. 14 reaction of the last step (dynamic samples only, else 0) */
+    SPH_FIELD_RIGID_BODIES = 15,   /* SphRigidBody [n_bodies]                                rw */
+    SPH_FIELD_BOUNDARY_CELL_START = 16, /* int [n_cells+1] boundary grid */
+    SPH_FIELD_BOUNDARY_CELL_OF_PARTICLE = 17 /* int [n_boundary] */
+} SphField;
+
+typedef struct SphSim SphSim;
+
+/* Bytes of device workspace a simulation of this size needs (0 on invalid parameters). */
+size_t sph_workspace_bytes(const SphParams *params, int n_fluid, int n_boundary, int n_bodies);
+
+/* Grid geometry the library will use for these parameters (R11): dims[0..2] = n_x, n_y, n_z,
+ * dims[3] = n_cells.  Also the neighbour-list capacities after rounding: caps[0] = Kf, caps[1] = Kb. */
+int sph_grid_dims(const SphParams *params, int dims[4], int caps[2]);
+
+/* Create: copies the inputs into the workspace, builds the boundary grid, computes the Akinci
+ * volumes Psi_k = rho0 / sum_{k' in same body} W_kk' (Eq. 11, R9), builds the fluid
+ * grid.  `bodies` is a HOST array.  `cuda_stream` is a cudaStream_t (NULL = legacy default
+ * stream).  Synchronises the stream once.  On failure *out = NULL and the error text is
+ * available from sph_last_error(NULL). */
+int sph_create(const SphParams *params, const SphBuffers *buffers, int n_fluid, int n_boundary,
+               const SphRigidBody *bodies, int n_bodies, int cuda_device, void *cuda_stream,
+               SphSim **out);
+
+/* A1-A3 only: cell keys, histogram + exclusive prefix scan, counting-sort scatter and reorder of
+ * the particle store ("prefix sum"; R11, R12).  Leaves the store sorted.  Also
+ * builds the per-particle neighbour lists and rho, alpha (A4) so that every read field is
+ * consistent with the current positions. */
+int sph_build_grid(SphSim *sim);
+
+/* n_steps DFSPH steps (Alg. 1 PAPER.md:127-134 with the pressure solve of Alg. 2
+ * realised by DFSPH [5] = Eq. 8 and Eq. 10 sources): grid -> rho, alpha ->
+ * divergence-free solve -> non-pressure forces (gravity, Eq. 15 or Eq. 16-19) -> constant-density
+ * solve -> symplectic Euler -> rigid bodies.  Asynchronous, one CUDA-graph launch per step. */
+int sph_step_dfsph(SphSim *sim, int n_steps);
+
+/* n_steps WCSPH steps (PAPER.md:140 EOS; Eq. 7, 12, 13; R17): fixed work per step. */
+int sph_step_wcsph(SphSim *sim, int n_steps);
+
+/* Override the iteration counts of the next steps: -1 = tolerances decide, >= 0 = exactly that
+ * many iterations of the divergence solve / density solve / CG.  Takes effect without re-capture. */
+int sph_set_forced_iterations(SphSim *sim, int forced_v, int forced_d, int forced_cg);
+
+/* Copy one field out (un-permuted to original id order) / in.  `bytes` must equal the field's
+ * size.  is_host = 0: dst/src is a device pointer, copy is asynchronous on the stream;
+ * is_host = 1: host pointer, the call returns after the copy has completed.
+ * sph_write_state (any writable field) invalidates grid-derived fields until the next
+ * sph_build_grid / step. */
+int sph_read_state(SphSim *sim, int field, void *dst, size_t bytes, int is_host);
+int sph_write_state(SphSim *sim, int field, const void *src, size_t bytes, int is_host);
+
+/* The only call that always synchronises: copies the device statistics block to the host. */
+int sph_read_stats(SphSim *sim, SphStats *dst_host);
+
+/* Number of kernel launches (graph kernel nodes executed are counted per node per graph launch,
+ * loop bodies once per executed iteration) issued for this simulation since create. */
+long long sph_launch_count(SphSim *sim);
+
+const char *sph_last_error(const SphSim *sim);
+void sph_destroy(SphSim *sim);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

@@ -1,0 +1,810 @@
+// sph_api.cu -- host side of libsph_b200: workspace layout, step orchestration (one CUDA graph
+// per step with device-side WHILE loops) and the C ABI of include/sph.h.
+//
+// Product code.  It never includes, links or calls anything under oracle/.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "sph_common.cuh"
+#include "sph_grid.cuh"
+#include "sph_passes.cuh"
+#include "sph_rigid.cuh"
+
+using namespace sph;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Carver {             // carves 256-byte aligned sub-buffers out of the workspace
+    char *base;
+    size_t off = 0;
+    explicit Carver(void *b) : base(static_cast<char *>(b)) {}
+    template <typename T> T *take(size_t n)
+    {
+        size_t bytes = (n * sizeof(T) + 255) & ~size_t(255);
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += bytes;
+        return p;
+    }
+};
+
+struct GridBufs {           // one uniform grid over one particle set
+    int n = 0;
+    int *key = nullptr, *off = nullptr, *slot = nullptr;
+    int *cell_start = nullptr;      // [ncells + 1 (+ pad to 4)]
+    int *tile_sum = nullptr;
+    int ntiles = 0;
+};
+
+}  // namespace
+
+struct SphSim {
+    SphParams prm{};
+    SimConst c{};
+    int nbodies = 0, ndyn = 0;
+    int device = 0;
+    cudaStream_t stream = nullptr, cap_stream = nullptr;
+    int nblocks = 0;                // CTAs of the per-particle kernels (= number of partials)
+    size_t cs_len = 0;              // ncells + 1 rounded up to 4
+    // fluid store
+    float4 *posA = nullptr, *velA = nullptr, *posB = nullptr, *velB = nullptr, *velC = nullptr, *posk = nullptr;
+    int *idA = nullptr, *idB = nullptr;
+    float *alpha = nullptr;
+    GridBufs gf, gb;
+    int *nl_f = nullptr, *nl_b = nullptr, *ncount = nullptr;
+    float *partial = nullptr, *partial2 = nullptr;
+    float4 *cg_r = nullptr, *cg_p = nullptr, *cg_Ap = nullptr;
+    // boundary store
+    float4 *borig_pos = nullptr, *borig_vel = nullptr, *brest = nullptr, *bforce = nullptr;
+    float4 *bpos_s = nullptr, *bvel_s = nullptr;
+    int *bbody = nullptr, *bid_s = nullptr, *dyn_idx = nullptr;
+    SphRigidBody *bodies = nullptr;
+    DevControl *ctl = nullptr;
+    DevStats *stats = nullptr;
+    void *staging = nullptr;
+    size_t staging_bytes = 0;
+    // host
+    int *pinned = nullptr;          // small pinned block (loop predicate, stats)
+    bool derived_valid = false;     // B-order fields (rho, alpha, lists, cell_start) match the store
+    cudaGraphExec_t exec[2] = { nullptr, nullptr };   // 0 DFSPH, 1 WCSPH
+    long long fixed_nodes[2] = { 0, 0 };
+    long long body_nodes[2][3] = { { 0, 0, 0 }, { 0, 0, 0 } };
+    long long graph_steps[2] = { 0, 0 };              // graph launches per method (host view)
+    long long misc_launches = 0;
+    long long *cur_counter = nullptr;
+    std::string err;
+};
+
+namespace {
+
+#define CUDA_TRY(sim, expr)                                                                     \
+    do {                                                                                        \
+        cudaError_t e_ = (expr);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            char b_[512];                                                                       \
+            snprintf(b_, sizeof b_, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            (sim)->err = b_;                                                                    \
+            return SPH_ECUDA;                                                                   \
+        }                                                                                       \
+    } while (0)
+
+#define LAUNCH(sim, kern, grid, block, strm, ...)                                               \
+    do {                                                                                        \
+        kern<<<(grid), (block), 0, (strm)>>>(__VA_ARGS__);                                      \
+        ++*(sim)->cur_counter;                                                                  \
+        CUDA_TRY(sim, cudaGetLastError());                                                      \
+    } while (0)
+
+inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+// Grid geometry, reading R11 (restated here; the oracle has its own copy of this definition).
+bool make_geom(const SphParams &p, Geom &g, std::string &why)
+{
+    float h = p.support_radius;
+    if (!(h > 0.f)) { why = "support_radius must be > 0"; return false; }
+    float cedge = h * 1.0009765625f;
+    g.inv_c = 1.0f / cedge;
+    g.ox = p.domain_min[0]; g.oy = p.domain_min[1]; g.oz = p.domain_min[2];
+    long long n[3];
+    for (int a = 0; a < 3; ++a) {
+        float ext = p.domain_max[a] - p.domain_min[a];
+        if (!(ext >= 0.f)) { why = "domain_max < domain_min"; return false; }
+        float t = floorf(ext * g.inv_c);
+        if (!(t < 2.0e9f)) { why = "grid too large"; return false; }
+        n[a] = (long long)t + 1;
+        if (n[a] < 1) n[a] = 1;
+    }
+    long long nc = n[0] * n[1] * n[2];
+    if (nc > 2000000000LL) { why = "grid exceeds 2^31 cells"; return false; }
+    g.nx = (int)n[0]; g.ny = (int)n[1]; g.nz = (int)n[2]; g.ncells = (int)nc;
+    return true;
+}
+
+int list_cap(int v) { if (v <= 0) v = 64; v = (v + 3) & ~3; if (v > 65532) v = 65532; return v; }
+
+bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &why)
+{
+    if (nf < 0 || nb < 0) { why = "negative particle count"; return false; }
+    if (!(p.particle_radius > 0.f) || !(p.rest_density > 0.f) || !(p.dt > 0.f)) {
+        why = "particle_radius, rest_density and dt must be > 0"; return false;
+    }
+    if (!make_geom(p, c.g, why)) return false;
+    c.nf = nf; c.nb = nb;
+    c.kf = list_cap(p.max_fluid_neighbors);
+    c.kb = list_cap(p.max_boundary_neighbors);
+    c.h = p.support_radius;
+    c.h2 = c.h * c.h;                                   // fp32 product (R10)
+    c.inv_h = 1.0f / c.h;
+    double hd = (double)p.support_radius;
+    double sigma = 8.0 / (3.14159265358979323846 * hd * hd * hd);   // R1
+    c.sigma = (float)sigma;
+    c.grad_c = (float)(sigma / hd);
+    double d = 2.0 * (double)p.particle_radius;
+    c.m = p.particle_mass > 0.f ? p.particle_mass : (float)((double)p.rest_density * d * d * d);   // R3
+    c.rho0 = p.rest_density; c.dt = p.dt;
+    c.gx = p.gravity[0]; c.gy = p.gravity[1]; c.gz = p.gravity[2];
+    c.nu = p.kinematic_viscosity;
+    c.mu = p.kinematic_viscosity * p.rest_density;      // R21
+    c.visc_eps = (float)(0.01 * hd * hd);
+    c.wc_k = p.wcsph_stiffness; c.wc_gamma = p.wcsph_exponent;
+    c.has_dynamic = 0;
+    return true;
+}
+
+// Workspace layout: fills the simulation's pointers when base != NULL, returns the bytes needed.
+size_t layout(SphSim &s, void *base)
+{
+    Carver w(base);
+    const size_t nf = (size_t)s.c.nf, nb = (size_t)s.c.nb;
+    const size_t nf1 = nf ? nf : 1, nb1 = nb ? nb : 1;
+    s.cs_len = ((size_t)s.c.g.ncells + 1 + 3) & ~size_t(3);
+    s.nblocks = cdiv((long long)nf1, kBlock);
+    const size_t nwarps = (nf1 + 31) / 32;
+    s.ctl = w.take<DevControl>(1);
+    s.stats = w.take<DevStats>(1);
+    s.posA = w.take<float4>(nf1); s.velA = w.take<float4>(nf1); s.idA = w.take<int>(nf1);
+    s.posB = w.take<float4>(nf1); s.velB = w.take<float4>(nf1); s.idB = w.take<int>(nf1);
+    s.velC = s.prm.viscosity_mode == 1 ? w.take<float4>(nf1) : nullptr;
+    s.posk = w.take<float4>(nf1);
+    s.alpha = w.take<float>(nf1);
+    s.gf.n = (int)nf;
+    s.gf.key = w.take<int>(nf1); s.gf.off = w.take<int>(nf1); s.gf.slot = w.take<int>(nf1);
+    s.gf.cell_start = w.take<int>(s.cs_len);
+    s.gf.ntiles = cdiv((long long)s.cs_len, kScanTile);
+    s.gf.tile_sum = w.take<int>((size_t)s.gf.ntiles);
+    s.nl_f = w.take<int>(nwarps * (size_t)s.c.kf * 32);
+    s.nl_b = w.take<int>(nwarps * (size_t)s.c.kb * 32);
+    s.ncount = w.take<int>(nf1);
+    s.partial = w.take<float>((size_t)s.nblocks);
+    s.partial2 = w.take<float>((size_t)s.nblocks);
+    if (s.prm.viscosity_mode == 2) {
+        s.cg_r = w.take<float4>(nf1); s.cg_p = w.take<float4>(nf1); s.cg_Ap = w.take<float4>(nf1);
+    }
+    s.borig_pos = w.take<float4>(nb1); s.borig_vel = w.take<float4>(nb1);
+    s.brest = w.take<float4>(nb1); s.bforce = w.take<float4>(nb1);
+    s.bpos_s = w.take<float4>(nb1); s.bvel_s = w.take<float4>(nb1);
+    s.bbody = w.take<int>(nb1); s.bid_s = w.take<int>(nb1); s.dyn_idx = w.take<int>(nb1);
+    s.gb.n = (int)nb;
+    s.gb.key = w.take<int>(nb1); s.gb.off = w.take<int>(nb1); s.gb.slot = w.take<int>(nb1);
+    s.gb.cell_start = w.take<int>(s.cs_len);
+    s.gb.ntiles = s.gf.ntiles;
+    s.gb.tile_sum = w.take<int>((size_t)s.gb.ntiles);
+    s.bodies = w.take<SphRigidBody>((size_t)(s.nbodies > 0 ? s.nbodies : 1));
+    size_t st = 16 * (nf1 > nb1 ? nf1 : nb1);
+    if (st < 4 * s.cs_len) st = 4 * s.cs_len;
+    if (st < sizeof(SphRigidBody) * (size_t)(s.nbodies + 1)) st = sizeof(SphRigidBody) * (size_t)(s.nbodies + 1);
+    s.staging_bytes = st;
+    s.staging = w.take<char>(st);
+    return w.off;
+}
+
+// ------------------------------------------------------------------------------------------
+// A1-A3 on one particle set: keys + histogram, scan, scatter, canonical reorder.
+int enqueue_grid(SphSim *s, cudaStream_t st, GridBufs &g, const float4 *a_in, const float4 *b_in,
+                 const int *id_in, float4 *a_out, float4 *b_out, int *id_out, int *oob)
+{
+    CUDA_TRY(s, cudaMemsetAsync(g.cell_start, 0, s->cs_len * sizeof(int), st));
+    if (g.n > 0)
+        LAUNCH(s, k_cell_key_hist, cdiv(g.n, 256), 256, st, a_in, g.n, s->c.g, g.key, g.off, g.cell_start, oob);
+    const int nscan = s->c.g.ncells + 1;
+    LAUNCH(s, k_scan_tile_sums, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
+    LAUNCH(s, k_scan_tile_offsets, 1, 1024, st, g.tile_sum, g.ntiles);
+    LAUNCH(s, k_scan_apply, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
+    if (g.n > 0) {
+        LAUNCH(s, k_scatter_slots, cdiv(g.n, 256), 256, st, g.key, g.off, g.cell_start, g.n, g.slot);
+        LAUNCH(s, k_reorder, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
+               a_out, b_out, id_out);
+    }
+    return SPH_OK;
+}
+
+PassCtx make_ctx(const SphSim *s)
+{
+    PassCtx p;
+    p.c = s->c;
+    p.pos = s->posB; p.bpos = s->bpos_s;
+    p.fcs = s->gf.cell_start; p.bcs = s->gb.cell_start;
+    p.nl_f = s->nl_f; p.nl_b = s->nl_b; p.ncount = s->ncount;
+    return p;
+}
+
+int enqueue_boundary_grid(SphSim *s, cudaStream_t st)
+{
+    return enqueue_grid(s, st, s->gb, s->borig_pos, s->borig_vel, nullptr, s->bpos_s, s->bvel_s, s->bid_s, nullptr);
+}
+
+int enqueue_fluid_grid_and_density(SphSim *s, cudaStream_t st)
+{
+    int rc = enqueue_grid(s, st, s->gf, s->posA, s->velA, s->idA, s->posB, s->velB, s->idB, &s->stats->oob);
+    if (rc) return rc;
+    if (s->c.nf > 0) {
+        PassCtx p = make_ctx(s);
+        if (s->prm.use_neighbor_list)
+            LAUNCH(s, k_density_alpha<true>, s->nblocks, kBlock, st, p, s->velB, s->alpha, &s->stats->lc);
+        else
+            LAUNCH(s, k_density_alpha<false>, s->nblocks, kBlock, st, p, s->velB, s->alpha, &s->stats->lc);
+    }
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Solver loops.  graph mode: a conditional WHILE node whose body is captured on the helper
+// stream; host mode: the host reads the predicate after every iteration.
+struct LoopCtx {
+    cudaStream_t st;
+    cudaGraphConditionalHandle h;
+    int use_handle;
+};
+
+int read_cont(SphSim *s, int *cont)
+{
+    CUDA_TRY(s, cudaMemcpyAsync(s->pinned, &s->ctl->cont, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    *cont = s->pinned[0];
+    return SPH_OK;
+}
+
+template <class Init, class Body>
+int run_loop(SphSim *s, bool graph_mode, long long *body_counter, Init init, Body body)
+{
+    if (!graph_mode) {
+        LoopCtx lc{ s->stream, 0, 0 };
+        int rc = init(lc);
+        if (rc) return rc;
+        int cont = 0;
+        if ((rc = read_cont(s, &cont))) return rc;
+        while (cont) {
+            if ((rc = body(lc))) return rc;
+            if ((rc = read_cont(s, &cont))) return rc;
+        }
+        return SPH_OK;
+    }
+    cudaStreamCaptureStatus status;
+    cudaGraph_t graph = nullptr;
+    const cudaGraphNode_t *deps = nullptr;
+    size_t ndeps = 0;
+    CUDA_TRY(s, cudaStreamGetCaptureInfo_v2(s->stream, &status, nullptr, &graph, &deps, &ndeps));
+    if (status != cudaStreamCaptureStatusActive) { s->err = "run_loop: stream is not capturing"; return SPH_ESTATE; }
+    cudaGraphConditionalHandle handle;
+    CUDA_TRY(s, cudaGraphConditionalHandleCreate(&handle, graph, 0, 0));
+    LoopCtx top{ s->stream, handle, 1 };
+    int rc = init(top);                  // captured into the parent graph; sets the first predicate
+    if (rc) return rc;
+    CUDA_TRY(s, cudaStreamGetCaptureInfo_v2(s->stream, &status, nullptr, &graph, &deps, &ndeps));
+    cudaGraphNodeParams np = { cudaGraphNodeTypeConditional };
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeWhile;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    CUDA_TRY(s, cudaGraphAddNode(&node, graph, deps, ndeps, &np));
+    cudaGraph_t body_graph = np.conditional.phGraph_out[0];
+    CUDA_TRY(s, cudaStreamUpdateCaptureDependencies(s->stream, &node, 1, cudaStreamSetCaptureDependencies));
+    CUDA_TRY(s, cudaStreamBeginCaptureToGraph(s->cap_stream, body_graph, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+    long long *saved = s->cur_counter;
+    s->cur_counter = body_counter;
+    LoopCtx in{ s->cap_stream, handle, 1 };
+    rc = body(in);
+    s->cur_counter = saved;
+    cudaGraph_t dummy = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->cap_stream, &dummy);
+    if (rc) return rc;
+    CUDA_TRY(s, e);
+    return SPH_OK;
+}
+
+template <bool LIST>
+int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+{
+    PassCtx p = make_ctx(s);
+    const bool dyn = s->c.has_dynamic != 0;
+    if (mode == MODE_DIV) {
+        if (dyn) LAUNCH(s, (k_solver_p<LIST, MODE_DIV, true>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
+        else     LAUNCH(s, (k_solver_p<LIST, MODE_DIV, false>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
+    } else {
+        if (dyn) LAUNCH(s, (k_solver_p<LIST, MODE_DENS, true>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
+        else     LAUNCH(s, (k_solver_p<LIST, MODE_DENS, false>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
+    }
+    LAUNCH(s, k_solver_c<LIST>, s->nblocks, kBlock, lc.st, p, s->posk, vel);
+    if (dyn && s->ndyn > 0)
+        LAUNCH(s, k_boundary_force, cdiv(s->ndyn, kBlock), kBlock, lc.st, s->c, s->dyn_idx, s->ndyn, s->borig_pos,
+               s->posk, s->gf.cell_start, s->bforce);
+    if (mode == MODE_DIV)
+        LAUNCH(s, k_solver_ctrl<MODE_DIV>, 1, 256, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+    else
+        LAUNCH(s, k_solver_ctrl<MODE_DENS>, 1, 256, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+    return SPH_OK;
+}
+
+template <bool LIST>
+int enqueue_step_t(SphSim *s, int method, bool graph_mode)
+{
+    cudaStream_t st = s->stream;
+    const int nf = s->c.nf;
+    const bool dyn = s->c.has_dynamic != 0;
+    long long *bc = s->body_nodes[method];
+    LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl);
+    if (dyn) {
+        int rc = enqueue_boundary_grid(s, st);
+        if (rc) return rc;
+        CUDA_TRY(s, cudaMemsetAsync(s->bforce, 0, sizeof(float4) * (size_t)s->c.nb, st));
+    }
+    int rc = enqueue_fluid_grid_and_density(s, st);
+    if (rc) return rc;
+    float4 *vcur = s->velB;
+    if (nf > 0) {
+        PassCtx p = make_ctx(s);
+        if (method == 0) {
+            // divergence-free solve (A5)
+            rc = run_loop(s, graph_mode, &bc[LOOP_DIV],
+                [&](const LoopCtx &lc) -> int { LAUNCH(s, k_loop_init, 1, 1, lc.st, (int)LOOP_DIV, s->ctl, lc.h, lc.use_handle); return (int)SPH_OK; },
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->velB); });
+            if (rc) return rc;
+            // non-pressure accelerations (A6 / A11)
+            if (s->prm.viscosity_mode == 1) {
+                LAUNCH(s, k_explicit_viscosity<LIST>, s->nblocks, kBlock, st, p, s->velB, s->velC);
+                vcur = s->velC;
+            } else {
+                LAUNCH(s, k_gravity, cdiv(nf, 256), 256, st, s->c, s->velB, s->velB);
+                if (s->prm.viscosity_mode == 2) {
+                    rc = run_loop(s, graph_mode, &bc[LOOP_CG],
+                        [&](const LoopCtx &lc) -> int {
+                            LAUNCH(s, (k_cg_apply<LIST, true>), s->nblocks, kBlock, lc.st, p, s->velB, s->cg_r, s->cg_p, s->partial, s->partial2);
+                            LAUNCH(s, k_cg_ctrl0, 1, 256, lc.st, s->partial, s->partial2, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+                            return (int)SPH_OK;
+                        },
+                        [&](const LoopCtx &lc) -> int {
+                            LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, s->cg_p, s->cg_Ap, (float4 *)nullptr, s->partial, (float *)nullptr);
+                            LAUNCH(s, k_cg_ctrl1, 1, 256, lc.st, s->partial, s->nblocks, s->ctl);
+                            LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->velB, s->cg_r, s->partial2);
+                            LAUNCH(s, k_cg_ctrl2, 1, 256, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);
+                            LAUNCH(s, k_cg_direction, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_r, s->cg_p);
+                            return (int)SPH_OK;
+                        });
+                    if (rc) return rc;
+                }
+            }
+            // constant-density solve (A7)
+            rc = run_loop(s, graph_mode, &bc[LOOP_DENS],
+                [&](const LoopCtx &lc) -> int { LAUNCH(s, k_loop_init, 1, 1, lc.st, (int)LOOP_DENS, s->ctl, lc.h, lc.use_handle); return (int)SPH_OK; },
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur); });
+            if (rc) return rc;
+        } else {
+            // WCSPH (A10)
+            LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->velB, s->posk);
+            if (s->prm.viscosity_mode == 1) {
+                LAUNCH(s, k_explicit_viscosity<LIST>, s->nblocks, kBlock, st, p, s->velB, s->velC);
+                vcur = s->velC;
+            } else {
+                LAUNCH(s, k_gravity, cdiv(nf, 256), 256, st, s->c, s->velB, s->velB);
+            }
+            LAUNCH(s, k_solver_c<LIST>, s->nblocks, kBlock, st, p, s->posk, vcur);
+            if (dyn && s->ndyn > 0)
+                LAUNCH(s, k_boundary_force, cdiv(s->ndyn, kBlock), kBlock, st, s->c, s->dyn_idx, s->ndyn, s->borig_pos,
+                       s->posk, s->gf.cell_start, s->bforce);
+        }
+        LAUNCH(s, k_integrate, cdiv(nf, 256), 256, st, s->c, s->posB, vcur, s->idB, s->posA, s->velA, s->idA,
+               &s->stats->vmax_bits, &s->stats->nan_count);
+    }
+    if (dyn && s->nbodies > 0)
+        LAUNCH(s, k_rigid_step, s->nbodies, 256, st, s->c, s->bodies, s->prm.tank_min[0], s->prm.tank_min[1],
+               s->prm.tank_min[2], s->prm.tank_max[0], s->prm.tank_max[1], s->prm.tank_max[2], s->brest, s->bforce,
+               s->borig_pos, s->borig_vel);
+    LAUNCH(s, k_step_end, 1, 1, st, s->stats);
+    return SPH_OK;
+}
+
+int enqueue_step(SphSim *s, int method, bool graph_mode)
+{
+    return s->prm.use_neighbor_list ? enqueue_step_t<true>(s, method, graph_mode)
+                                    : enqueue_step_t<false>(s, method, graph_mode);
+}
+
+int build_graph(SphSim *s, int method)
+{
+    long long fixed = 0;
+    s->cur_counter = &fixed;
+    s->body_nodes[method][0] = s->body_nodes[method][1] = s->body_nodes[method][2] = 0;
+    cudaError_t e = cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) { s->cur_counter = &s->misc_launches; CUDA_TRY(s, e); }
+    int rc = enqueue_step(s, method, true);
+    cudaGraph_t graph = nullptr;
+    e = cudaStreamEndCapture(s->stream, &graph);
+    s->cur_counter = &s->misc_launches;
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    CUDA_TRY(s, e);
+    cudaGraphExec_t exec = nullptr;
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    CUDA_TRY(s, e);
+    s->exec[method] = exec;
+    s->fixed_nodes[method] = fixed;
+    return SPH_OK;
+}
+
+int do_steps(SphSim *s, int method, int n_steps)
+{
+    if (!s) return SPH_EINVAL;
+    if (n_steps < 0) { s->err = "n_steps < 0"; return SPH_EINVAL; }
+    DeviceGuard dg(s->device);
+    if (s->prm.use_cuda_graph) {
+        if (!s->exec[method]) {
+            int rc = build_graph(s, method);
+            if (rc) return rc;
+        }
+        for (int k = 0; k < n_steps; ++k) CUDA_TRY(s, cudaGraphLaunch(s->exec[method], s->stream));
+        s->graph_steps[method] += n_steps;
+    } else {
+        for (int k = 0; k < n_steps; ++k) {
+            int rc = enqueue_step(s, method, false);
+            if (rc) return rc;
+        }
+    }
+    if (n_steps > 0) s->derived_valid = true;
+    return SPH_OK;
+}
+
+struct FieldInfo { size_t bytes; bool writable; bool derived; };
+
+bool field_info(const SphSim *s, int field, FieldInfo &fi)
+{
+    const size_t nf = (size_t)s->c.nf, nb = (size_t)s->c.nb, nc1 = (size_t)s->c.g.ncells + 1;
+    switch (field) {
+    case SPH_FIELD_POS: case SPH_FIELD_VEL: fi = { nf * 12, true, false }; return true;
+    case SPH_FIELD_DENSITY: case SPH_FIELD_ALPHA: case SPH_FIELD_KAPPA_OVER_RHO: fi = { nf * 4, false, true }; return true;
+    case SPH_FIELD_CELL_START: fi = { nc1 * 4, false, true }; return true;
+    case SPH_FIELD_CELL_OF_PARTICLE: case SPH_FIELD_SORTED_ID: fi = { nf * 4, false, true }; return true;
+    case SPH_FIELD_NEIGHBOR_COUNT: fi = { nf * 8, false, true }; return true;
+    case SPH_FIELD_FLUID_NEIGHBORS: fi = { nf * (size_t)s->c.kf * 4, false, true }; return true;
+    case SPH_FIELD_BOUNDARY_NEIGHBORS: fi = { nf * (size_t)s->c.kb * 4, false, true }; return true;
+    case SPH_FIELD_BOUNDARY_POS: case SPH_FIELD_BOUNDARY_VEL: fi = { nb * 12, true, false }; return true;
+    case SPH_FIELD_BOUNDARY_PSI: fi = { nb * 4, false, false }; return true;
+    case SPH_FIELD_BOUNDARY_FORCE: fi = { nb * 12, false, false }; return true;
+    case SPH_FIELD_RIGID_BODIES: fi = { sizeof(SphRigidBody) * (size_t)s->nbodies, true, false }; return true;
+    case SPH_FIELD_BOUNDARY_CELL_START: fi = { nc1 * 4, false, false }; return true;
+    case SPH_FIELD_BOUNDARY_CELL_OF_PARTICLE: fi = { nb * 4, false, false }; return true;
+    default: return false;
+    }
+}
+
+// writes the field into a DEVICE buffer `out` (asynchronously on the stream)
+int export_field(SphSim *s, int field, void *out, size_t bytes)
+{
+    cudaStream_t st = s->stream;
+    const int nf = s->c.nf, nb = s->c.nb;
+    if (bytes == 0) return SPH_OK;
+    switch (field) {
+    case SPH_FIELD_POS: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->posA, s->idA, nf, (float *)out); break;
+    case SPH_FIELD_VEL: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->velA, s->idA, nf, (float *)out); break;
+    case SPH_FIELD_DENSITY: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->velB, s->idB, nf, (float *)out); break;
+    case SPH_FIELD_ALPHA: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->alpha, s->idB, nf, (float *)out); break;
+    case SPH_FIELD_KAPPA_OVER_RHO: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posk, s->idB, nf, (float *)out); break;
+    case SPH_FIELD_CELL_START:
+        CUDA_TRY(s, cudaMemcpyAsync(out, s->gf.cell_start, bytes, cudaMemcpyDeviceToDevice, st)); break;
+    case SPH_FIELD_BOUNDARY_CELL_START:
+        CUDA_TRY(s, cudaMemcpyAsync(out, s->gb.cell_start, bytes, cudaMemcpyDeviceToDevice, st)); break;
+    case SPH_FIELD_CELL_OF_PARTICLE:
+        LAUNCH(s, k_export_keys, cdiv(nf, 256), 256, st, s->posB, s->idB, nf, s->c.g, (int *)out); break;
+    case SPH_FIELD_BOUNDARY_CELL_OF_PARTICLE:
+        LAUNCH(s, k_export_keys, cdiv(nb, 256), 256, st, s->bpos_s, s->bid_s, nb, s->c.g, (int *)out); break;
+    case SPH_FIELD_SORTED_ID:
+        CUDA_TRY(s, cudaMemcpyAsync(out, s->idB, bytes, cudaMemcpyDeviceToDevice, st)); break;
+    case SPH_FIELD_NEIGHBOR_COUNT: LAUNCH(s, k_export_counts, cdiv(nf, 256), 256, st, s->ncount, s->idB, nf, (int *)out); break;
+    case SPH_FIELD_FLUID_NEIGHBORS:
+        LAUNCH(s, k_export_neighbors, cdiv((long long)nf * s->c.kf, 256), 256, st, s->nl_f, s->ncount, 0, s->idB, s->idB, nf, s->c.kf, (int *)out); break;
+    case SPH_FIELD_BOUNDARY_NEIGHBORS:
+        LAUNCH(s, k_export_neighbors, cdiv((long long)nf * s->c.kb, 256), 256, st, s->nl_b, s->ncount, 16, s->idB, s->bid_s, nf, s->c.kb, (int *)out); break;
+    case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->borig_pos, (const int *)nullptr, nb, (float *)out); break;
+    case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->borig_vel, (const int *)nullptr, nb, (float *)out); break;
+    case SPH_FIELD_BOUNDARY_PSI: LAUNCH(s, k_export_w, cdiv(nb, 256), 256, st, s->borig_pos, (const int *)nullptr, nb, (float *)out); break;
+    case SPH_FIELD_BOUNDARY_FORCE: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->bforce, (const int *)nullptr, nb, (float *)out); break;
+    case SPH_FIELD_RIGID_BODIES:
+        CUDA_TRY(s, cudaMemcpyAsync(out, s->bodies, bytes, cudaMemcpyDeviceToDevice, st)); break;
+    default: s->err = "unknown field"; return SPH_EINVAL;
+    }
+    return SPH_OK;
+}
+
+int import_field(SphSim *s, int field, const void *src, size_t bytes)
+{
+    cudaStream_t st = s->stream;
+    const int nf = s->c.nf, nb = s->c.nb;
+    if (bytes == 0) return SPH_OK;
+    switch (field) {
+    case SPH_FIELD_POS: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->posA); break;
+    case SPH_FIELD_VEL: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->velA); break;
+    case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_pos); break;
+    case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_vel); break;
+    case SPH_FIELD_RIGID_BODIES:
+        CUDA_TRY(s, cudaMemcpyAsync(s->bodies, src, bytes, cudaMemcpyDeviceToDevice, st)); break;
+    default: s->err = "field is not writable"; return SPH_EINVAL;
+    }
+    return SPH_OK;
+}
+
+}  // namespace
+
+// ==============================================================================================
+extern "C" {
+
+size_t sph_workspace_bytes(const SphParams *params, int n_fluid, int n_boundary, int n_bodies)
+{
+    if (!params || n_bodies < 0) return 0;
+    SphSim tmp;
+    tmp.prm = *params;
+    tmp.nbodies = n_bodies;
+    std::string why;
+    if (!make_const(*params, n_fluid, n_boundary, tmp.c, why)) return 0;
+    return layout(tmp, nullptr);
+}
+
+int sph_grid_dims(const SphParams *params, int dims[4], int caps[2])
+{
+    if (!params) return SPH_EINVAL;
+    Geom g;
+    std::string why;
+    if (!make_geom(*params, g, why)) return SPH_EDOMAIN;
+    if (dims) { dims[0] = g.nx; dims[1] = g.ny; dims[2] = g.nz; dims[3] = g.ncells; }
+    if (caps) { caps[0] = list_cap(params->max_fluid_neighbors); caps[1] = list_cap(params->max_boundary_neighbors); }
+    return SPH_OK;
+}
+
+int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int n_boundary,
+               const SphRigidBody *bodies, int n_bodies, int cuda_device, void *cuda_stream, SphSim **out)
+{
+    if (out) *out = nullptr;
+    if (!params || !buf || !out || n_bodies < 0 || (n_bodies > 0 && !bodies)) { g_create_error = "null argument"; return SPH_EINVAL; }
+    SphSim *s = new SphSim;
+    s->prm = *params;
+    s->nbodies = n_bodies;
+    s->device = cuda_device;
+    s->stream = static_cast<cudaStream_t>(cuda_stream);
+    s->cur_counter = &s->misc_launches;
+    auto fail = [&](int code) { g_create_error = s->err; if (s->cap_stream) cudaStreamDestroy(s->cap_stream); if (s->pinned) cudaFreeHost(s->pinned); delete s; return code; };
+    if (!make_const(*params, n_fluid, n_boundary, s->c, s->err)) return fail(s->err.find("grid") != std::string::npos ? SPH_EDOMAIN : SPH_EINVAL);
+    if (n_fluid > 0 && (!buf->fluid_pos || !buf->fluid_vel)) { s->err = "fluid_pos / fluid_vel is NULL"; return fail(SPH_EINVAL); }
+    if (n_boundary > 0 && (!buf->boundary_pos || !buf->boundary_body)) { s->err = "boundary_pos / boundary_body is NULL"; return fail(SPH_EINVAL); }
+    if (params->use_cuda_graph && s->stream == nullptr) { s->err = "use_cuda_graph needs a created stream: CUDA graphs cannot be captured on the legacy default stream"; return fail(SPH_EINVAL); }
+    if (n_boundary > 0 && n_bodies == 0) { s->err = "boundary particles need at least one body"; return fail(SPH_EINVAL); }
+    std::vector<int> dyn;
+    for (int b = 0; b < n_bodies; ++b) {
+        const SphRigidBody &B = bodies[b];
+        if (B.first_particle < 0 || B.n_particles < 0 || B.first_particle + B.n_particles > n_boundary) { s->err = "body particle range out of bounds"; return fail(SPH_EINVAL); }
+        if (B.dynamic) {
+            if (!(B.mass > 0.f) || !(B.inertia_body[0] > 0.f) || !(B.inertia_body[1] > 0.f) || !(B.inertia_body[2] > 0.f)) { s->err = "dynamic body needs positive mass and inertia"; return fail(SPH_EINVAL); }
+            s->c.has_dynamic = 1;
+            for (int k = 0; k < B.n_particles; ++k) dyn.push_back(B.first_particle + k);
+        }
+    }
+    s->ndyn = (int)dyn.size();
+    size_t need = layout(*s, nullptr);
+    if (!buf->workspace || buf->workspace_bytes < need) {
+        char b[160]; snprintf(b, sizeof b, "workspace too small: need %zu bytes, got %zu", need, buf->workspace_bytes);
+        s->err = b; return fail(SPH_ENOMEM);
+    }
+    if ((reinterpret_cast<uintptr_t>(buf->workspace) & 255) != 0) { s->err = "workspace must be 256-byte aligned"; return fail(SPH_EINVAL); }
+    layout(*s, buf->workspace);
+
+    DeviceGuard dg(s->device);
+    auto run = [&]() -> int {
+        cudaStream_t st = s->stream;
+        CUDA_TRY(s, cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+        CUDA_TRY(s, cudaMallocHost(&s->pinned, 4096));
+        const int nf = s->c.nf, nb = s->c.nb;
+        // control + statistics blocks
+        DevControl hc;
+        memset(&hc, 0, sizeof hc);
+        const SphParams &p = s->prm;
+        hc.forced_v = p.force_iterations ? p.min_iter_divergence : -1;
+        hc.forced_d = p.force_iterations ? p.min_iter_density : -1;
+        hc.forced_cg = -1;
+        hc.min_v = p.min_iter_divergence; hc.max_v = p.max_iter_divergence;
+        hc.min_d = p.min_iter_density; hc.max_d = p.max_iter_density;
+        hc.max_cg = p.cg_max_iter; hc.enable_div = p.enable_divergence_solve;
+        hc.eta_v = p.eta_divergence; hc.eta_d = p.eta_density; hc.cg_tol = p.cg_rel_tol;
+        memcpy(s->pinned, &hc, sizeof hc);
+        CUDA_TRY(s, cudaMemcpyAsync(s->ctl, s->pinned, sizeof hc, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(s, cudaMemsetAsync(s->stats, 0, sizeof(DevStats), st));
+        // fluid store, original order; ids = identity
+        if (nf > 0) {
+            LAUNCH(s, k_pack_vec3, cdiv(nf, 256), 256, st, buf->fluid_pos, nf, s->posA, 0.f);
+            LAUNCH(s, k_pack_vec3, cdiv(nf, 256), 256, st, buf->fluid_vel, nf, s->velA, 0.f);
+            LAUNCH(s, k_iota, cdiv(nf, 256), 256, st, s->idA, nf);
+        }
+        // boundary store
+        if (s->nbodies > 0) {
+            CUDA_TRY(s, cudaStreamSynchronize(st));       // pinned block is reused below
+            if (sizeof(SphRigidBody) * (size_t)s->nbodies <= 4096) {
+                memcpy(s->pinned, bodies, sizeof(SphRigidBody) * (size_t)s->nbodies);
+                CUDA_TRY(s, cudaMemcpyAsync(s->bodies, s->pinned, sizeof(SphRigidBody) * (size_t)s->nbodies, cudaMemcpyHostToDevice, st));
+                CUDA_TRY(s, cudaStreamSynchronize(st));
+            } else {
+                CUDA_TRY(s, cudaMemcpy(s->bodies, bodies, sizeof(SphRigidBody) * (size_t)s->nbodies, cudaMemcpyHostToDevice));
+            }
+        }
+        CUDA_TRY(s, cudaMemsetAsync(s->gb.cell_start, 0, s->cs_len * sizeof(int), st));
+        if (nb > 0) {
+            LAUNCH(s, k_pack_vec3, cdiv(nb, 256), 256, st, buf->boundary_pos, nb, s->borig_pos, 0.f);
+            CUDA_TRY(s, cudaMemcpyAsync(s->bbody, buf->boundary_body, sizeof(int) * (size_t)nb, cudaMemcpyDeviceToDevice, st));
+            CUDA_TRY(s, cudaMemsetAsync(s->bforce, 0, sizeof(float4) * (size_t)nb, st));
+            if (s->ndyn > 0) CUDA_TRY(s, cudaMemcpy(s->dyn_idx, dyn.data(), sizeof(int) * dyn.size(), cudaMemcpyHostToDevice));
+            LAUNCH(s, k_body_rest, cdiv(nb, 256), 256, st, s->borig_pos, s->bbody, s->bodies, nb, s->brest, s->borig_vel);
+            int rc = enqueue_boundary_grid(s, st);
+            if (rc) return rc;
+            LAUNCH(s, k_boundary_psi, cdiv(nb, kBlock), kBlock, st, s->c, s->bpos_s, s->bid_s, s->gb.cell_start, s->bbody, s->borig_pos);
+        }
+        CUDA_TRY(s, cudaStreamSynchronize(st));
+        return SPH_OK;
+    };
+    int rc = run();
+    if (rc) return fail(rc);
+    rc = sph_build_grid(s);
+    if (rc) return fail(rc);
+    cudaError_t e = cudaStreamSynchronize(s->stream);
+    if (e != cudaSuccess) { s->err = std::string("sph_create: ") + cudaGetErrorString(e); return fail(SPH_ECUDA); }
+    *out = s;
+    return SPH_OK;
+}
+
+int sph_build_grid(SphSim *s)
+{
+    if (!s) return SPH_EINVAL;
+    DeviceGuard dg(s->device);
+    cudaStream_t st = s->stream;
+    LAUNCH(s, k_list_counters_reset, 1, 1, st, s->stats);
+    if (s->c.has_dynamic) {
+        int rc = enqueue_boundary_grid(s, st);
+        if (rc) return rc;
+    }
+    int rc = enqueue_fluid_grid_and_density(s, st);
+    if (rc) return rc;
+    // leave the persistent store sorted as well (the next step's sort is then the identity)
+    const size_t nf = (size_t)s->c.nf;
+    if (nf > 0) {
+        CUDA_TRY(s, cudaMemcpyAsync(s->posA, s->posB, nf * sizeof(float4), cudaMemcpyDeviceToDevice, st));
+        CUDA_TRY(s, cudaMemcpyAsync(s->velA, s->velB, nf * sizeof(float4), cudaMemcpyDeviceToDevice, st));
+        CUDA_TRY(s, cudaMemcpyAsync(s->idA, s->idB, nf * sizeof(int), cudaMemcpyDeviceToDevice, st));
+        // posk mirrors the positions with kappa/rho = 0 until a solver pass writes it
+        CUDA_TRY(s, cudaMemcpyAsync(s->posk, s->posA, nf * sizeof(float4), cudaMemcpyDeviceToDevice, st));
+    }
+    s->derived_valid = true;
+    return SPH_OK;
+}
+
+int sph_step_dfsph(SphSim *s, int n_steps) { return do_steps(s, 0, n_steps); }
+int sph_step_wcsph(SphSim *s, int n_steps) { return do_steps(s, 1, n_steps); }
+
+int sph_set_forced_iterations(SphSim *s, int forced_v, int forced_d, int forced_cg)
+{
+    if (!s) return SPH_EINVAL;
+    DeviceGuard dg(s->device);
+    // the three ints are the first members of DevControl
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    s->pinned[0] = forced_v; s->pinned[1] = forced_d; s->pinned[2] = forced_cg;
+    CUDA_TRY(s, cudaMemcpyAsync(s->ctl, s->pinned, 3 * sizeof(int), cudaMemcpyHostToDevice, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return SPH_OK;
+}
+
+int sph_read_state(SphSim *s, int field, void *dst, size_t bytes, int is_host)
+{
+    if (!s) return SPH_EINVAL;
+    FieldInfo fi;
+    if (!field_info(s, field, fi)) { s->err = "unknown field"; return SPH_EINVAL; }
+    if (bytes != fi.bytes) { char b[128]; snprintf(b, sizeof b, "field %d is %zu bytes, caller passed %zu", field, fi.bytes, bytes); s->err = b; return SPH_EINVAL; }
+    if (bytes > 0 && !dst) { s->err = "dst is NULL"; return SPH_EINVAL; }
+    if (fi.derived && !s->derived_valid) { s->err = "field is stale: call sph_build_grid or a step first"; return SPH_ESTATE; }
+    DeviceGuard dg(s->device);
+    if (!is_host) return export_field(s, field, dst, bytes);
+    if (bytes > s->staging_bytes) { s->err = "field too large for a host read; read it into a device buffer"; return SPH_EINVAL; }
+    int rc = export_field(s, field, s->staging, bytes);
+    if (rc) return rc;
+    if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(dst, s->staging, bytes, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return SPH_OK;
+}
+
+int sph_write_state(SphSim *s, int field, const void *src, size_t bytes, int is_host)
+{
+    if (!s) return SPH_EINVAL;
+    FieldInfo fi;
+    if (!field_info(s, field, fi) || !fi.writable) { s->err = "field is not writable"; return SPH_EINVAL; }
+    if (bytes != fi.bytes) { char b[128]; snprintf(b, sizeof b, "field %d is %zu bytes, caller passed %zu", field, fi.bytes, bytes); s->err = b; return SPH_EINVAL; }
+    if (bytes > 0 && !src) { s->err = "src is NULL"; return SPH_EINVAL; }
+    DeviceGuard dg(s->device);
+    int rc;
+    if (is_host) {
+        if (bytes > s->staging_bytes) { s->err = "field too large for a host write"; return SPH_EINVAL; }
+        if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging, src, bytes, cudaMemcpyHostToDevice, s->stream));
+        rc = import_field(s, field, s->staging, bytes);
+        if (rc) return rc;
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    } else {
+        rc = import_field(s, field, src, bytes);
+        if (rc) return rc;
+    }
+    s->derived_valid = false;
+    return SPH_OK;
+}
+
+int sph_read_stats(SphSim *s, SphStats *o)
+{
+    if (!s || !o) return SPH_EINVAL;
+    DeviceGuard dg(s->device);
+    DevStats *h = reinterpret_cast<DevStats *>(s->pinned + 64);
+    CUDA_TRY(s, cudaMemcpyAsync(h, s->stats, sizeof(DevStats), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    memset(o, 0, sizeof *o);
+    o->steps_done = h->steps_done; o->total_it_v = h->total_it_v; o->total_it_d = h->total_it_d;
+    o->total_cg_iters = h->total_cg;
+    o->it_v = h->it_v; o->it_d = h->it_d; o->cg_iters = h->cg_iters;
+    o->err_v = h->err_v; o->err_rho = h->err_rho; o->cg_residual = h->cg_residual;
+    o->oob_count = h->oob; o->overflow_count = h->lc.overflow; o->nan_count = h->nan_count;
+    o->max_iter_hit = h->max_iter_hit;
+    unsigned vb = h->vmax_bits; float vm; memcpy(&vm, &vb, 4); o->v_max = vm;
+    o->max_fluid_neighbors = h->lc.max_f; o->max_boundary_neighbors = h->lc.max_b;
+    o->mean_fluid_neighbors = s->c.nf > 0 ? (float)((double)h->lc.sum_f / (double)s->c.nf) : 0.f;
+    return SPH_OK;
+}
+
+long long sph_launch_count(SphSim *s)
+{
+    if (!s) return 0;
+    long long n = s->misc_launches;
+    if (s->prm.use_cuda_graph && (s->graph_steps[0] + s->graph_steps[1]) > 0) {
+        SphStats st;
+        if (sph_read_stats(s, &st) != SPH_OK) return n;
+        // loop bodies: iterations are only recorded per solver, not per method; a simulation
+        // normally uses one method, so attribute them to the method that has run
+        int m = s->graph_steps[0] > 0 ? 0 : 1;
+        n += s->graph_steps[0] * s->fixed_nodes[0] + s->graph_steps[1] * s->fixed_nodes[1];
+        n += st.total_it_v * s->body_nodes[m][LOOP_DIV] + st.total_it_d * s->body_nodes[m][LOOP_DENS] +
+             st.total_cg_iters * s->body_nodes[m][LOOP_CG];
+    }
+    return n;
+}
+
+const char *sph_last_error(const SphSim *s) { return s ? s->err.c_str() : g_create_error.c_str(); }
+
+void sph_destroy(SphSim *s)
+{
+    if (!s) return;
+    DeviceGuard dg(s->device);
+    cudaStreamSynchronize(s->stream);
+    for (int m = 0; m < 2; ++m) if (s->exec[m]) cudaGraphExecDestroy(s->exec[m]);
+    if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
+    if (s->pinned) cudaFreeHost(s->pinned);
+    delete s;
+}
+
+}  // extern "C"

@@ -1,0 +1,165 @@
+// sph_common.cuh -- shared device-side definitions of libsph_b200 (sm_100a).
+//
+// Product code: shares nothing with oracle/ (the CPU fp64 test oracle).  Citations are
+// /root/reference/PAPER.md line numbers and the readings Rn of DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sph.h"
+
+namespace sph {
+
+constexpr int kBlock = 128;        // threads per CTA of the per-particle kernels
+constexpr int kWarp = 32;
+constexpr int kBigCell = 2048;     // cells above this size keep atomic order (R12 note in DESIGN.md)
+
+// Uniform grid geometry (reading R11): cell edge c = h (1 + 2^-10) in fp32, origin = domain_min,
+// n_a = floor((max_a - o_a) * inv_c) + 1, linear key x-fastest.
+struct Geom {
+    float ox, oy, oz, inv_c;
+    int nx, ny, nz, ncells;
+};
+
+// Per-simulation constants handed to kernels by value.
+struct SimConst {
+    Geom g;
+    int nf, nb;          // fluid / boundary particle counts
+    int kf, kb;          // neighbour-list capacities (rows per warp tile)
+    float h, h2, inv_h;  // support radius, h*h in fp32 (R10), 1/h
+    float sigma;         // 8 / (pi h^3)           (R1)
+    float grad_c;        // sigma / h
+    float m;             // fluid particle mass     (R3)
+    float rho0, dt;
+    float gx, gy, gz;
+    float nu, mu;        // kinematic / dynamic viscosity (mu = nu rho0, R21)
+    float visc_eps;      // 0.01 h^2                (Eq. 15 / 19, R4)
+    float wc_k, wc_gamma;
+    int has_dynamic;     // any dynamic rigid body
+};
+
+// Loop-control block in device memory (one per simulation).  Written by the host only through
+// cudaMemcpyAsync on the simulation's stream (sph_set_forced_iterations).
+struct DevControl {
+    int forced_v, forced_d, forced_cg;   // -1: tolerances decide
+    int min_v, max_v, min_d, max_d, max_cg;
+    int enable_div;
+    float eta_v, eta_d, cg_tol;
+    // running state of the current step
+    int cont;                            // loop predicate as last evaluated (host-driven mode reads it)
+    int it;                              // iteration counter of the running loop
+    double cg_bb, cg_rr, cg_alpha, cg_beta;
+    int cg_break;
+};
+
+// Statistics block in device memory; sph_read_stats copies it out and converts to SphStats.
+struct ListCounters {
+    int overflow, max_f, max_b, pad;
+    unsigned long long sum_f;
+};
+struct DevStats {
+    long long steps_done, total_it_v, total_it_d, total_cg;
+    int it_v, it_d, cg_iters, max_iter_hit;
+    float err_v, err_rho, cg_residual;
+    int oob, nan_count;
+    unsigned vmax_bits;
+    ListCounters lc;
+};
+
+// ---------------------------------------------------------------------------------------------
+// Cell coordinate of one point: (int)floorf((x - o) * inv_c) with separate fp32 subtract and
+// multiply (no contraction), clamped into [0, n-1]; NaN goes to cell 0 (R11).
+__device__ __forceinline__ int cell_coord(float x, float o, float inv_c, int n, bool &clamped)
+{
+    float t = __fmul_rn(__fsub_rn(x, o), inv_c);
+    if (!(t == t)) { clamped = true; return 0; }
+    if (t < 0.0f) { clamped = true; return 0; }
+    if (t >= (float)n) { clamped = true; return n - 1; }
+    return (int)floorf(t);
+}
+
+__device__ __forceinline__ int cell_key(const Geom &g, float x, float y, float z, bool &clamped,
+                                        int &cx, int &cy, int &cz)
+{
+    clamped = false;
+    cx = cell_coord(x, g.ox, g.inv_c, g.nx, clamped);
+    cy = cell_coord(y, g.oy, g.inv_c, g.ny, clamped);
+    cz = cell_coord(z, g.oz, g.inv_c, g.nz, clamped);
+    return cx + g.nx * (cy + g.ny * cz);
+}
+
+// Squared distance of reading R10: d2 = fma(dz, dz, fma(dy, dy, dx*dx)), every operation in
+// binary32 with round-to-nearest and exactly this association, so that the strict predicate
+// d2 < h2 selects bit-identical neighbour sets on every implementation.
+__device__ __forceinline__ float dist2_r10(float dx, float dy, float dz)
+{
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+
+// Cubic spline with support radius h (R1): W = sigma { 6(q^3 - q^2) + 1, q <= 1/2 ; 2(1-q)^3, q <= 1 }.
+// Returns w(q) WITHOUT sigma (callers scale the finished sum once).
+__device__ __forceinline__ float spline_w(float q)
+{
+    float t = 1.0f - q;
+    float a = fmaf(6.0f * q * q, q - 1.0f, 1.0f);
+    float b = 2.0f * t * t * t;
+    return q <= 0.5f ? a : b;
+}
+
+// Gradient factor f with grad_i W(x_i - x_j) = sigma/h * f * (x_i - x_j):
+//   q <= 1/2: w'(q)/r = 6 q (3q - 2) / r = 6 (3q - 2) / h      (no division, finite at r = 0)
+//   q <= 1  : w'(q)/r = -6 (1 - q)^2 / r
+// (R1, R2: the product with d = 0 vanishes at zero distance).  rinv = 1/r (unused when q <= 1/2).
+__device__ __forceinline__ float spline_gradf(float q, float rinv, float inv_h)
+{
+    float t = 1.0f - q;
+    float a = 6.0f * fmaf(3.0f, q, -2.0f) * inv_h;
+    float b = -6.0f * t * t * rinv;
+    return q <= 0.5f ? a : b;
+}
+
+// r and 1/r from d2 (d2 > 0 for the second branch; guarded for d2 == 0).
+__device__ __forceinline__ void r_and_rinv(float d2, float &r, float &rinv)
+{
+    rinv = rsqrtf(fmaxf(d2, 1e-30f));
+    r = d2 * rinv;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Block-wide sums (warp shuffle, then one shared-memory hop).  Result valid in thread 0.
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ float warp_max(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+template <typename T>
+__device__ __forceinline__ T block_sum(T v, T *smem /* >= blockDim/32 */)
+{
+    v = warp_sum(v);
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (lane == 0) smem[w] = v;
+    __syncthreads();
+    T r = T(0);
+    if (w == 0) {
+        r = lane < nw ? smem[lane] : T(0);
+        r = warp_sum(r);
+    }
+    return r;
+}
+
+}  // namespace sph

@@ -1,0 +1,193 @@
+// sph_grid.cuh -- A1-A3: cell keys + histogram, exclusive prefix scan, counting-sort scatter,
+// canonical intra-cell order and reorder of the particle store.
+//
+// The paper only says that its neighbour structure is built with a prefix sum;
+// geometry, linearisation and clamping are reading R11, the order inside a cell reading R12.
+#pragma once
+#include "sph_common.cuh"
+
+namespace sph {
+
+// A1 + first half of A2: key[i] = linear cell of pos[i]; off[i] = arrival rank inside the cell
+// (atomic, NOT deterministic -- k_reorder canonicalises); count[key]++; clamps counted per warp.
+__global__ void __launch_bounds__(256)
+k_cell_key_hist(const float4 *__restrict__ pos, int n, Geom g, int *__restrict__ key,
+                int *__restrict__ off, int *__restrict__ count, int *__restrict__ oob)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool clamped = false;
+    if (i < n) {
+        float4 p = pos[i];
+        int cx, cy, cz;
+        int k = cell_key(g, p.x, p.y, p.z, clamped, cx, cy, cz);
+        key[i] = k;
+        off[i] = atomicAdd(&count[k], 1);
+    }
+    unsigned b = __ballot_sync(0xffffffffu, clamped);
+    if (oob != nullptr && b != 0u && (threadIdx.x & 31) == 0) atomicAdd(oob, __popc(b));
+}
+
+// keys only (SPH_FIELD_CELL_OF_PARTICLE export): out[id[s]] = key of sorted slot s.
+__global__ void __launch_bounds__(256)
+k_export_keys(const float4 *__restrict__ pos, const int *__restrict__ id, int n, Geom g,
+              int *__restrict__ out)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    float4 p = pos[s];
+    bool clamped; int cx, cy, cz;
+    out[id[s]] = cell_key(g, p.x, p.y, p.z, clamped, cx, cy, cz);
+}
+
+// ---------------------------------------------------------------------------------------------
+// A2: exclusive prefix scan of count[0 .. n) in place (n = ncells + 1, count[ncells] = 0 so that
+// the last entry becomes N).  Three launches: tile sums, scan of tile sums, tile rescan.
+constexpr int kScanThreads = 256;
+constexpr int kScanRounds = 4;                                  // int4 per thread per round
+constexpr int kScanTile = kScanThreads * 4 * kScanRounds;       // 4096 cells per CTA
+
+__device__ __forceinline__ int4 load_int4_guard(const int *a, int base, int n)
+{
+    if (base + 3 < n) return *reinterpret_cast<const int4 *>(a + base);
+    int4 v = make_int4(0, 0, 0, 0);
+    if (base < n) v.x = a[base];
+    if (base + 1 < n) v.y = a[base + 1];
+    if (base + 2 < n) v.z = a[base + 2];
+    return v;
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_tile_sums(const int *__restrict__ a, int n, int *__restrict__ tile_sum)
+{
+    __shared__ int sm[kScanThreads / 32];
+    int base = blockIdx.x * kScanTile;
+    int s = 0;
+#pragma unroll
+    for (int r = 0; r < kScanRounds; ++r) {
+        int4 v = load_int4_guard(a, base + r * kScanThreads * 4 + threadIdx.x * 4, n);
+        s += v.x + v.y + v.z + v.w;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int t = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) t += sm[w];
+        tile_sum[blockIdx.x] = t;
+    }
+}
+
+// block-wide exclusive scan of one int per thread; returns exclusive prefix, *total = block sum
+__device__ __forceinline__ int block_excl_scan(int v, int *sm /* [blockDim/32 + 1] */, int *total)
+{
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();
+    if (lane == 31) sm[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int x = lane < nw ? sm[lane] : 0;
+        int xi = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, xi, o);
+            if (lane >= o) xi += t;
+        }
+        if (lane < nw) sm[lane] = xi - x;   // exclusive warp offsets
+        if (lane == 31) sm[32] = xi;        // total (nw <= 32)
+    }
+    __syncthreads();
+    *total = sm[32];
+    return sm[w] + inc - v;
+}
+
+__global__ void __launch_bounds__(1024)
+k_scan_tile_offsets(int *__restrict__ tile_sum, int ntiles)
+{
+    __shared__ int sm[33];
+    int carry = 0;
+    for (int base = 0; base < ntiles; base += 1024) {
+        int i = base + threadIdx.x;
+        int v = i < ntiles ? tile_sum[i] : 0;
+        int total;
+        int ex = block_excl_scan(v, sm, &total);
+        if (i < ntiles) tile_sum[i] = carry + ex;
+        carry += total;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_scan_apply(int *__restrict__ a, int n, const int *__restrict__ tile_off)
+{
+    __shared__ int sm[33];
+    int base = blockIdx.x * kScanTile;
+    int carry = tile_off[blockIdx.x];
+#pragma unroll 1
+    for (int r = 0; r < kScanRounds; ++r) {
+        int e = base + r * kScanThreads * 4 + threadIdx.x * 4;
+        int4 v = load_int4_guard(a, e, n);
+        int t = v.x + v.y + v.z + v.w;
+        int total;
+        int ex = block_excl_scan(t, sm, &total) + carry;
+        int4 o;
+        o.x = ex; o.y = ex + v.x; o.z = o.y + v.y; o.w = o.z + v.z;
+        if (e + 3 < n) *reinterpret_cast<int4 *>(a + e) = o;
+        else {
+            if (e < n) a[e] = o.x;
+            if (e + 1 < n) a[e + 1] = o.y;
+            if (e + 2 < n) a[e + 2] = o.z;
+        }
+        carry += total;
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// A3 first half: slot[cell_start[key] + off] = source index.
+__global__ void __launch_bounds__(256)
+k_scatter_slots(const int *__restrict__ key, const int *__restrict__ off,
+                const int *__restrict__ cell_start, int n, int *__restrict__ slot_src)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    slot_src[cell_start[key[i]] + off[i]] = i;
+}
+
+// A3 second half: canonical order inside a cell = ascending source index (= order of the
+// previous sorted store, R12: makes the run bit-reproducible although the histogram atomics are
+// not), then gather of every persistent field into sorted order.
+// For the fluid store: a = pos(x,y,z,-), b = vel(vx,vy,vz,-), ids carried.
+// For the boundary store: a = (x,y,z,psi), b = (vx,vy,vz,-), ids = original boundary index.
+__global__ void __launch_bounds__(256)
+k_reorder(const int *__restrict__ slot_src, const int *__restrict__ key,
+          const int *__restrict__ cell_start, int n,
+          const float4 *__restrict__ a_in, const float4 *__restrict__ b_in,
+          const int *__restrict__ id_in, float4 *__restrict__ a_out, float4 *__restrict__ b_out,
+          int *__restrict__ id_out)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int src = slot_src[s];
+    int k = key[src];
+    int cs = cell_start[k], ce = cell_start[k + 1];
+    int rank;
+    if (ce - cs > kBigCell) rank = s - cs;       // degenerate pile-up: keep arrival order
+    else {
+        rank = 0;
+        for (int t = cs; t < ce; ++t) rank += (slot_src[t] < src) ? 1 : 0;
+    }
+    int dst = cs + rank;
+    a_out[dst] = a_in[src];
+    if (b_in != nullptr) b_out[dst] = b_in[src];
+    id_out[dst] = id_in != nullptr ? id_in[src] : src;
+}
+
+}  // namespace sph

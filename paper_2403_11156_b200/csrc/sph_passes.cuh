@@ -1,0 +1,457 @@
+// sph_passes.cuh -- A4-A7, A9-A12: the neighbour-sum kernels, their device-side reductions and
+// loop control.
+//
+// Store layout (all fp32, sorted cell order, one thread per fluid particle):
+//   pos [nf] float4  x, y, z, -
+//   vel [nf] float4  vx, vy, vz, rho        (rho_i rides in .w: the viscosity sums need rho_j)
+//   posk[nf] float4  x, y, z, kappa_i/rho_i (written by every P-pass, gathered by the C-pass:
+//                                            one 16-byte gather per neighbour instead of two)
+//   bpos[nb] float4  x, y, z, Psi           bvel[nb] float4 vx, vy, vz, -
+// Neighbour lists (built once per step by k_density_alpha, consumed by every later pass):
+//   warp tile w = i / 32 owns rows [w*K*32, (w+1)*K*32); entry k of particle i is at
+//   tile + k*32 + (i & 31), so that a warp reads row k with one coalesced 128-byte load.
+#pragma once
+#include "sph_common.cuh"
+
+namespace sph {
+
+struct PassCtx {
+    SimConst c;
+    const float4 *pos;
+    const float4 *bpos;
+    const int *fcs;     // fluid cell_start [ncells + 1]
+    const int *bcs;     // boundary cell_start
+    int *nl_f, *nl_b;   // neighbour lists
+    int *ncount;        // [nf] (#fluid) | (#boundary << 16)
+};
+
+// ---------------------------------------------------------------------------------------------
+// Candidate enumeration: the 27 cells around (cx, cy, cz) as 9 x-runs.  Cells are linearised
+// x-fastest and the store is sorted by cell, so the three x-adjacent cells of one (y, z) row are
+// ONE contiguous index range [cell_start[row + x0], cell_start[row + x1 + 1]).
+template <class F>
+__device__ __forceinline__ void for_each_candidate(const Geom &g, const int *__restrict__ cs,
+                                                   int cx, int cy, int cz, F &&f)
+{
+    int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.nx - 1);
+#pragma unroll 1
+    for (int dz = -1; dz <= 1; ++dz) {
+        int z = cz + dz;
+        if ((unsigned)z >= (unsigned)g.nz) continue;
+#pragma unroll 1
+        for (int dy = -1; dy <= 1; ++dy) {
+            int y = cy + dy;
+            if ((unsigned)y >= (unsigned)g.ny) continue;
+            int row = g.nx * (y + g.ny * z);
+            int s = __ldg(cs + row + x0), e = __ldg(cs + row + x1 + 1);
+#pragma unroll 4
+            for (int j = s; j < e; ++j) f(j);
+        }
+    }
+}
+
+// Visit every neighbour of fluid particle i (sorted index), fluid first then boundary:
+//   ff(j, pj, dx, dy, dz, d2) for fluid j != i with d2 < h2,  fb(k, pk, dx, dy, dz, d2) for boundary k;
+//   d = x_i - x_j in fp32, d2 as in reading R10.
+// LIST = true : gather through the per-step list (predicate was evaluated when it was built);
+// LIST = false: walk the cells and evaluate the predicate.
+// `src` is the float4 array whose xyz are the neighbour positions and whose .w the caller wants
+// (pos or posk); WITH_B = false skips the boundary part.
+template <bool LIST, bool WITH_B, class FF, class FB>
+__device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4 *__restrict__ src,
+                                                  int i, float xi, float yi, float zi, FF &&ff, FB &&fb)
+{
+    if (LIST) {
+        int packed = p.ncount[i];
+        int cf = packed & 0xffff, cb = (packed >> 16) & 0xffff;
+        const int *lf = p.nl_f + (size_t)(i >> 5) * p.c.kf * 32 + (i & 31);
+#pragma unroll 4
+        for (int k = 0; k < cf; ++k) {
+            int j = __ldg(lf + k * 32);
+            float4 q = __ldg(src + j);
+            float dx = xi - q.x, dy = yi - q.y, dz = zi - q.z;
+            ff(j, q, dx, dy, dz, dist2_r10(dx, dy, dz));
+        }
+        if (WITH_B && cb > 0) {
+            const int *lb = p.nl_b + (size_t)(i >> 5) * p.c.kb * 32 + (i & 31);
+#pragma unroll 2
+            for (int k = 0; k < cb; ++k) {
+                int j = __ldg(lb + k * 32);
+                float4 q = __ldg(p.bpos + j);
+                float dx = xi - q.x, dy = yi - q.y, dz = zi - q.z;
+                fb(j, q, dx, dy, dz, dist2_r10(dx, dy, dz));
+            }
+        }
+    } else {
+        bool cl; int cx, cy, cz;
+        cell_key(p.c.g, xi, yi, zi, cl, cx, cy, cz);
+        const float h2 = p.c.h2;
+        for_each_candidate(p.c.g, p.fcs, cx, cy, cz, [&](int j) {
+            float4 q = __ldg(src + j);
+            float dx = __fsub_rn(xi, q.x), dy = __fsub_rn(yi, q.y), dz = __fsub_rn(zi, q.z);
+            float d2 = dist2_r10(dx, dy, dz);
+            if (d2 < h2 && j != i) ff(j, q, dx, dy, dz, d2);
+        });
+        if (WITH_B && p.c.nb > 0) {
+            for_each_candidate(p.c.g, p.bcs, cx, cy, cz, [&](int j) {
+                float4 q = __ldg(p.bpos + j);
+                float dx = __fsub_rn(xi, q.x), dy = __fsub_rn(yi, q.y), dz = __fsub_rn(zi, q.z);
+                float d2 = dist2_r10(dx, dy, dz);
+                if (d2 < h2) fb(j, q, dx, dy, dz, d2);
+            });
+        }
+    }
+}
+
+// gradient factor for a pair at squared distance d2: grad_i W_ij = grad_c * gf * d
+__device__ __forceinline__ float pair_gradf(const SimConst &c, float d2)
+{
+    float r, rinv;
+    r_and_rinv(d2, r, rinv);
+    return spline_gradf(r * c.inv_h, rinv, c.inv_h);
+}
+
+// ---------------------------------------------------------------------------------------------
+// A4: density (Eq. 4 + Eq. 12; self term included, R2) and the DFSPH factor
+// alpha_i = rho_i / (|S_i|^2 + T_i), S_i = sum_j m gradW_ij + sum_k Psi_k gradW_ik,
+// T_i = sum_j |m gradW_ij|^2 (R5, R7), in ONE walk of the 27 cells that also writes the
+// neighbour lists every later pass of the step gathers through.
+template <bool WRITE_LIST>
+__global__ void __launch_bounds__(kBlock)
+k_density_alpha(PassCtx p, float4 *__restrict__ vel, float *__restrict__ alpha,
+                ListCounters *__restrict__ lc)
+{
+    const SimConst &c = p.c;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int cf = 0, cb = 0;
+    if (i < c.nf) {
+        float4 xi = p.pos[i];
+        float sw = 0.f, sx = 0.f, sy = 0.f, sz = 0.f, t2 = 0.f;    // fluid: sum w, sum gf d, sum gf^2 d2
+        float bw = 0.f, bx = 0.f, by = 0.f, bz = 0.f;              // boundary, Psi-weighted
+        int *lf = p.nl_f + (size_t)(i >> 5) * c.kf * 32 + (i & 31);
+        int *lb = p.nl_b + (size_t)(i >> 5) * c.kb * 32 + (i & 31);
+        for_each_neighbor<false, true>(p, p.pos, i, xi.x, xi.y, xi.z,
+            [&](int j, float4, float dx, float dy, float dz, float d2) {
+                float r, rinv;
+                r_and_rinv(d2, r, rinv);
+                float q = r * c.inv_h;
+                sw += spline_w(q);
+                float gf = spline_gradf(q, rinv, c.inv_h);
+                sx = fmaf(gf, dx, sx); sy = fmaf(gf, dy, sy); sz = fmaf(gf, dz, sz);
+                t2 = fmaf(gf * gf, d2, t2);
+                if (WRITE_LIST && cf < c.kf) lf[cf * 32] = j;
+                ++cf;
+            },
+            [&](int k, float4 pk, float dx, float dy, float dz, float d2) {
+                float r, rinv;
+                r_and_rinv(d2, r, rinv);
+                float q = r * c.inv_h;
+                bw = fmaf(pk.w, spline_w(q), bw);
+                float gf = pk.w * spline_gradf(q, rinv, c.inv_h);
+                bx = fmaf(gf, dx, bx); by = fmaf(gf, dy, by); bz = fmaf(gf, dz, bz);
+                if (WRITE_LIST && cb < c.kb) lb[cb * 32] = k;
+                ++cb;
+            });
+        float rho = c.sigma * fmaf(c.m, 1.0f + sw, bw);            // W(0) = sigma
+        float Sx = c.grad_c * fmaf(c.m, sx, bx), Sy = c.grad_c * fmaf(c.m, sy, by),
+              Sz = c.grad_c * fmaf(c.m, sz, bz);
+        float T = (c.grad_c * c.m) * (c.grad_c * c.m) * t2;
+        float den = fmaf(Sx, Sx, fmaf(Sy, Sy, fmaf(Sz, Sz, T)));
+        alpha[i] = den > 1e-6f ? rho / den : 0.0f;
+        vel[i].w = rho;
+        p.ncount[i] = min(cf, c.kf) | (min(cb, c.kb) << 16);
+    }
+    // statistics: overflow count, maxima, mean neighbour count (warp-aggregated atomics)
+    bool ovf = (i < c.nf) && (cf > c.kf || cb > c.kb);
+    unsigned bo = __ballot_sync(0xffffffffu, ovf);
+    int mf = cf, mb = cb, sf = cf;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mf = max(mf, __shfl_xor_sync(0xffffffffu, mf, o));
+        mb = max(mb, __shfl_xor_sync(0xffffffffu, mb, o));
+        sf += __shfl_xor_sync(0xffffffffu, sf, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (bo) atomicAdd(&lc->overflow, __popc(bo));
+        atomicMax(&lc->max_f, mf);
+        atomicMax(&lc->max_b, mb);
+        atomicAdd(&lc->sum_f, (unsigned long long)sf);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// P-pass of both solvers (A5 / A7).  Density rate (Eq. 6 times rho):
+//   D_i = sum_j m (v_i - v_j).gradW_ij + sum_k Psi_k (v_i - v_k).gradW_ik
+// DIV  (Eq. 10 source; R15): R_i = max(D_i, 0), kappa^v_i = alpha_i R_i / dt, term = R_i
+// DENS (Eq. 8-9; R15) : E_i = max(rho_i + dt D_i, rho0) - rho0,
+//                                          kappa_i = alpha_i E_i / dt^2, term = E_i
+// Writes posk[i] = (x_i, kappa_i / rho_i) and one partial sum of `term` per CTA.
+enum { MODE_DIV = 0, MODE_DENS = 1 };
+
+template <bool LIST, int MODE, bool DYN>
+__global__ void __launch_bounds__(kBlock)
+k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__ bvel,
+           const float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial)
+{
+    __shared__ float red[kBlock / 32];
+    const SimConst &c = p.c;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float term = 0.f;
+    if (i < c.nf) {
+        float4 xi = p.pos[i];
+        float4 vi = vel[i];
+        float df = 0.f, db = 0.f;
+        for_each_neighbor<LIST, true>(p, p.pos, i, xi.x, xi.y, xi.z,
+            [&](int j, float4, float dx, float dy, float dz, float d2) {
+                float4 vj = __ldg(vel + j);
+                float gf = pair_gradf(c, d2);
+                float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
+                df = fmaf(gf, dv, df);
+            },
+            [&](int k, float4 pk, float dx, float dy, float dz, float d2) {
+                float gf = pk.w * pair_gradf(c, d2);
+                float dv;
+                if (DYN) {
+                    float4 vk = __ldg(bvel + k);
+                    dv = fmaf(vi.x - vk.x, dx, fmaf(vi.y - vk.y, dy, (vi.z - vk.z) * dz));
+                } else dv = fmaf(vi.x, dx, fmaf(vi.y, dy, vi.z * dz));
+                db = fmaf(gf, dv, db);
+            });
+        float D = c.grad_c * fmaf(c.m, df, db);
+        float rho = vi.w, a = alpha[i], kappa;
+        if (MODE == MODE_DIV) {
+            term = fmaxf(D, 0.f);
+            kappa = a * term / c.dt;
+        } else {
+            term = fmaxf(fmaf(c.dt, D, rho), c.rho0) - c.rho0;
+            kappa = a * term / (c.dt * c.dt);
+        }
+        posk[i] = make_float4(xi.x, xi.y, xi.z, kappa / rho);
+    }
+    float s = block_sum(term, red);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+// C-pass (A5 / A7 / A10): pressure-like velocity update (Eq. 7 + Eq. 13 with p/rho^2 == kappa/rho,
+// PAPER.md:123, 200):  v_i -= dt [ sum_j m (kr_i + kr_j) gradW_ij + sum_k Psi_k kr_i gradW_ik ].
+template <bool LIST>
+__global__ void __launch_bounds__(kBlock)
+k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel)
+{
+    const SimConst &c = p.c;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.nf) return;
+    float4 xi = posk[i];
+    float kri = xi.w;
+    float fx = 0.f, fy = 0.f, fz = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
+    for_each_neighbor<LIST, true>(p, posk, i, xi.x, xi.y, xi.z,
+        [&](int, float4 pj, float dx, float dy, float dz, float d2) {
+            float s = (kri + pj.w) * pair_gradf(c, d2);
+            fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz);
+        },
+        [&](int, float4 pk, float dx, float dy, float dz, float d2) {
+            float s = pk.w * pair_gradf(c, d2);
+            bx = fmaf(s, dx, bx); by = fmaf(s, dy, by); bz = fmaf(s, dz, bz);
+        });
+    float4 v = vel[i];
+    float k = c.dt * c.grad_c;
+    v.x -= k * fmaf(c.m, fx, kri * bx);
+    v.y -= k * fmaf(c.m, fy, kri * by);
+    v.z -= k * fmaf(c.m, fz, kri * bz);
+    vel[i] = v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// A6, Alg. 1 l.1-2: v* = v + dt (g + a_visc).
+// mode 0 / 2: gravity only (elementwise; in place is fine).
+__global__ void __launch_bounds__(256)
+k_gravity(SimConst c, const float4 *__restrict__ vin, float4 *__restrict__ vout)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.nf) return;
+    float4 v = vin[i];
+    v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
+    vout[i] = v;
+}
+
+// mode 1: explicit viscosity, Eq. 15 (R4, R16, R22):
+//   a_i = nu 2(d+2) sum_j (m / rho_j) (v_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij, fluid-fluid only.
+// rho_j is vel[j].w (rho for DFSPH, the clamped rho~ for WCSPH).  Reads vin, writes vout != vin.
+template <bool LIST>
+__global__ void __launch_bounds__(kBlock)
+k_explicit_viscosity(PassCtx p, const float4 *__restrict__ vin, float4 *__restrict__ vout)
+{
+    const SimConst &c = p.c;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.nf) return;
+    float4 xi = p.pos[i];
+    float4 vi = vin[i];
+    float ax = 0.f, ay = 0.f, az = 0.f;
+    for_each_neighbor<LIST, false>(p, p.pos, i, xi.x, xi.y, xi.z,
+        [&](int j, float4, float dx, float dy, float dz, float d2) {
+            float4 vj = __ldg(vin + j);
+            float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
+            float s = pair_gradf(c, d2) * dv / ((d2 + c.visc_eps) * vj.w);
+            ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay); az = fmaf(s, dz, az);
+        },
+        [&](int, float4, float, float, float, float) {});
+    float k = c.dt * c.nu * 10.0f * c.m * c.grad_c;
+    vi.x += fmaf(c.dt, c.gx, k * ax);
+    vi.y += fmaf(c.dt, c.gy, k * ay);
+    vi.z += fmaf(c.dt, c.gz, k * az);
+    vout[i] = vi;
+}
+
+// ---------------------------------------------------------------------------------------------
+// A11: implicit viscosity (Eq. 16-19; R4, R21, R23), matrix-free CG on
+// (I - dt A) v* = v~ with
+//   (A u)_i = 2(d+2) sum_j mu m / (rho_i rho_j) (u_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij.
+// Vectors are float4 with rho in .w.  out_i = u_i - dt (A u)_i when RESIDUAL0 = false;
+// RESIDUAL0 = true is the start-up r0 = b - (I - dt A) b = dt A b (x0 = b = v~), which also seeds
+// the search direction and reduces |b|^2, |r0|^2.
+template <bool LIST, bool RESIDUAL0>
+__global__ void __launch_bounds__(kBlock)
+k_cg_apply(PassCtx p, const float4 *__restrict__ u, float4 *__restrict__ out,
+           float4 *__restrict__ out2, float *__restrict__ partial, float *__restrict__ partial2)
+{
+    __shared__ float red[kBlock / 32];
+    const SimConst &c = p.c;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float t1 = 0.f, t2 = 0.f;
+    if (i < c.nf) {
+        float4 xi = p.pos[i];
+        float4 ui = u[i];
+        float ax = 0.f, ay = 0.f, az = 0.f;
+        for_each_neighbor<LIST, false>(p, p.pos, i, xi.x, xi.y, xi.z,
+            [&](int j, float4, float dx, float dy, float dz, float d2) {
+                float4 uj = __ldg(u + j);
+                float du = fmaf(ui.x - uj.x, dx, fmaf(ui.y - uj.y, dy, (ui.z - uj.z) * dz));
+                float s = pair_gradf(c, d2) * du / ((d2 + c.visc_eps) * uj.w);
+                ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay); az = fmaf(s, dz, az);
+            },
+            [&](int, float4, float, float, float, float) {});
+        float k = c.dt * 10.0f * c.mu * c.m * c.grad_c / ui.w;     // dt * 2(d+2) mu m / rho_i
+        float Ax = k * ax, Ay = k * ay, Az = k * az;               // dt (A u)_i
+        if (RESIDUAL0) {
+            float4 r = make_float4(Ax, Ay, Az, ui.w);
+            out[i] = r;                                            // r0
+            out2[i] = r;                                           // p0 = r0
+            t1 = fmaf(ui.x, ui.x, fmaf(ui.y, ui.y, ui.z * ui.z));  // |b|^2
+            t2 = fmaf(Ax, Ax, fmaf(Ay, Ay, Az * Az));              // |r0|^2
+        } else {
+            float ox = ui.x - Ax, oy = ui.y - Ay, oz = ui.z - Az;  // (I - dt A) p
+            out[i] = make_float4(ox, oy, oz, ui.w);
+            t1 = fmaf(ui.x, ox, fmaf(ui.y, oy, ui.z * oz));        // p.Ap
+        }
+    }
+    float s1 = block_sum(t1, red);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s1;
+    if (RESIDUAL0) {
+        float s2 = block_sum(t2, red);
+        if (threadIdx.x == 0) partial2[blockIdx.x] = s2;
+    }
+}
+
+// x += a p;  r -= a Ap;  partial |r|^2
+__global__ void __launch_bounds__(256)
+k_cg_update(int n, const DevControl *__restrict__ ctl, const float4 *__restrict__ pd,
+            const float4 *__restrict__ Ap, float4 *__restrict__ x, float4 *__restrict__ r,
+            float *__restrict__ partial)
+{
+    __shared__ float red[8];
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float t = 0.f;
+    if (i < n) {
+        float a = (float)ctl->cg_alpha;
+        float4 pv = pd[i], av = Ap[i], xv = x[i], rv = r[i];
+        xv.x = fmaf(a, pv.x, xv.x); xv.y = fmaf(a, pv.y, xv.y); xv.z = fmaf(a, pv.z, xv.z);
+        rv.x = fmaf(-a, av.x, rv.x); rv.y = fmaf(-a, av.y, rv.y); rv.z = fmaf(-a, av.z, rv.z);
+        x[i] = xv; r[i] = rv;
+        t = fmaf(rv.x, rv.x, fmaf(rv.y, rv.y, rv.z * rv.z));
+    }
+    float s = block_sum(t, red);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+// p = r + beta p
+__global__ void __launch_bounds__(256)
+k_cg_direction(int n, const DevControl *__restrict__ ctl, const float4 *__restrict__ r,
+               float4 *__restrict__ pd)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float b = (float)ctl->cg_beta;
+    float4 rv = r[i], pv = pd[i];
+    pv.x = fmaf(b, pv.x, rv.x); pv.y = fmaf(b, pv.y, rv.y); pv.z = fmaf(b, pv.z, rv.z);
+    pd[i] = pv;
+}
+
+// ---------------------------------------------------------------------------------------------
+// A10: WCSPH equation of state (R17): rho~ = max(rho, rho0),
+// p = k((rho~/rho0)^gamma - 1), evaluated as k expm1(gamma log1p(delta)), delta = (rho~ - rho0)/rho0,
+// which keeps the small excess accurate in fp32.  posk.w = p / rho~^2, vel.w = rho~.
+__global__ void __launch_bounds__(256)
+k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, float4 *__restrict__ vel,
+            float4 *__restrict__ posk)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.nf) return;
+    float4 x = pos[i];
+    float rho = vel[i].w;
+    float rt = fmaxf(rho, c.rho0);
+    float delta = (rt - c.rho0) / c.rho0;
+    float pr = c.wc_k * expm1f(c.wc_gamma * log1pf(delta));
+    vel[i].w = rt;
+    posk[i] = make_float4(x.x, x.y, x.z, pr / (rt * rt));
+}
+
+// ---------------------------------------------------------------------------------------------
+// A9: symplectic Euler (Alg. 1 l.5-6): x += dt v with the already updated v.
+// Writes the persistent store (pos_out, vel_out, id_out) that the next step's sort reads, and the
+// step's v_max / non-finite counters.
+__global__ void __launch_bounds__(256)
+k_integrate(SimConst c, const float4 *__restrict__ pos, const float4 *__restrict__ vel,
+            const int *__restrict__ id, float4 *__restrict__ pos_out, float4 *__restrict__ vel_out,
+            int *__restrict__ id_out, unsigned *__restrict__ vmax_bits, int *__restrict__ nan_count)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float v2 = 0.f;
+    bool bad = false;
+    if (i < c.nf) {
+        float4 x = pos[i], v = vel[i];
+        x.x = fmaf(c.dt, v.x, x.x); x.y = fmaf(c.dt, v.y, x.y); x.z = fmaf(c.dt, v.z, x.z);
+        x.w = 0.f;
+        pos_out[i] = x;
+        vel_out[i] = make_float4(v.x, v.y, v.z, 0.f);
+        id_out[i] = id[i];
+        v2 = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
+        bad = !(isfinite(x.x) && isfinite(x.y) && isfinite(x.z) && isfinite(v2));
+        if (bad) v2 = 0.f;
+    }
+    v2 = warp_max(v2);
+    unsigned b = __ballot_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(vmax_bits, __float_as_uint(sqrtf(v2)));   // non-negative floats order like their bits
+        if (b) atomicAdd(nan_count, __popc(b));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// A12: loop control.  One CTA sums the per-CTA partials in a fixed order (fp64), evaluates the
+// loop predicate of Alg. 2 (R14: the error measured by this iteration's P-pass
+// is tested after its C-pass) and sets the CUDA-graph WHILE condition -- no host round trip.
+__device__ __forceinline__ double reduce_partials(const float *__restrict__ partial, int n, double *sm)
+{
+    double s = 0.0;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) s += (double)partial[k];
+    return block_sum(s, sm);
+}
+
+__device__ __forceinline__ void set_loop_condition(cudaGraphConditionalHandle h, int use_handle,
+                                                   DevControl *ctl, int cont)
+{
+    ctl->cont = cont;
+    if (use_handle) cudaGraphSetConditional(h, cont ? 1u : 0u);
+}
+
+}  // namespace sph

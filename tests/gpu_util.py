@@ -1,0 +1,108 @@
+"""Helpers of the GPU parity tests: drive the CUDA path (through the C ABI binding) and the
+fp64 oracle on the same seeded inputs and compare (protocol of DESIGN.md section 5 /
+SURVEY.md 8(c.5)).  Nothing here computes any SPH quantity itself."""
+from __future__ import annotations
+
+import numpy as np
+
+
+def np_(t):
+    return t.detach().cpu().numpy()
+
+
+def rows_to_sets(rows: np.ndarray):
+    """(n, K) int rows padded with -1 -> list of frozensets."""
+    return [frozenset(int(v) for v in r[r >= 0]) for r in rows]
+
+
+def csr_to_sets(start: np.ndarray, idx: np.ndarray):
+    return [frozenset(int(v) for v in idx[start[i]:start[i + 1]]) for i in range(len(start) - 1)]
+
+
+def make_pair(scene, oracle, **overrides):
+    """(gpu Sim, oracle Sim) on the same scene."""
+    from paper_2403_11156_b200 import binding
+    g = binding.Sim.from_scene(scene, **overrides)
+    o_over = {k: v for k, v in overrides.items()
+              if k not in ("max_fluid_neighbors", "max_boundary_neighbors", "use_cuda_graph", "use_neighbor_list")}
+    o = oracle.Sim.from_scene(scene, **o_over)
+    return g, o
+
+
+def assert_grid_parity(g, o):
+    """Bit-exact: cell_start, per-particle cell key, per-particle neighbour id sets."""
+    from paper_2403_11156_b200 import binding as B
+    g.sph_build_grid()
+    o.build_grid()
+    st = g.sph_read_stats()
+    assert st["overflow_count"] == 0, st
+    dims = o.grid_dims(0)
+    assert (g.nx, g.ny, g.nz, g.ncells) == tuple(dims)
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_OF_PARTICLE)), o.cell_of_particle(0))
+    assert st["oob_count"] == o.stats()["oob_count"]
+    if g.nb:
+        assert np.array_equal(np_(g.sph_read_state(B.BOUNDARY_CELL_START)), o.cell_start(1))
+        assert np.array_equal(np_(g.sph_read_state(B.BOUNDARY_CELL_OF_PARTICLE)), o.cell_of_particle(1))
+    cnt = np_(g.sph_read_state(B.NEIGHBOR_COUNT))
+    fs, fi = o.neighbors(0)
+    bs, bi = o.neighbors(1)
+    assert np.array_equal(cnt[:, 0], np.diff(fs))
+    assert np.array_equal(cnt[:, 1], np.diff(bs))
+    gf = rows_to_sets(np_(g.sph_read_state(B.FLUID_NEIGHBORS)))
+    assert gf == csr_to_sets(fs, fi)
+    gb = rows_to_sets(np_(g.sph_read_state(B.BOUNDARY_NEIGHBORS)))
+    assert gb == csr_to_sets(bs, bi)
+    # sorted ids are a permutation
+    sid = np_(g.sph_read_state(B.SORTED_ID))
+    assert np.array_equal(np.sort(sid), np.arange(g.nf))
+    return st
+
+
+def field_errors(g, o, scene, check_boundary=True):
+    """Normalised errors of rho, alpha (of the step's start), v, x after ONE step on both."""
+    from paper_2403_11156_b200 import binding as B
+    rho0 = scene.params["rest_density"]
+    gmag = float(np.linalg.norm(scene.params["gravity"]))
+    rho_g, rho_o = np_(g.sph_read_state(B.DENSITY)).astype(np.float64), o.density()
+    al_g, al_o = np_(g.sph_read_state(B.ALPHA)).astype(np.float64), o.alpha()
+    v_g, v_o = np_(g.sph_read_state(B.VEL)).astype(np.float64), o.vel()
+    x_g, x_o = np_(g.sph_read_state(B.POS)).astype(np.float64), o.pos()
+    vscale = max(float(np.linalg.norm(v_o, axis=1).max()), np.sqrt(gmag * scene.fluid_height), 1e-30)
+    dv = np.linalg.norm(v_g - v_o, axis=1)
+    e = dict(
+        rho=float(np.abs(rho_g - rho_o).max() / rho0),
+        alpha=float(np.abs(al_g - al_o).max() / max(np.abs(al_o).max(), 1e-300)),
+        vel=float(dv.max() / vscale),
+        vel_unfloored=float(dv.max() / max(float(np.linalg.norm(v_o, axis=1).max()), 1e-30)),
+        pos_abs=float(np.abs(x_g - x_o).max()),
+        vscale=vscale,
+    )
+    return e
+
+
+def sync_oracle_to_gpu(g, o, scene):
+    """Copy the GPU's fp32 state (fluid, boundary samples, bodies) into the oracle."""
+    from paper_2403_11156_b200 import binding as B
+    o.set_state(np_(g.sph_read_state(B.POS)), np_(g.sph_read_state(B.VEL)))
+    if g.nb and any(b.dynamic for b in scene.bodies):
+        o.set_boundary_state(np_(g.sph_read_state(B.BOUNDARY_POS)), np_(g.sph_read_state(B.BOUNDARY_VEL)))
+        from paper_2403_11156_b200.scenes import Body
+        o.set_bodies([Body(**b) for b in g.read_bodies()])
+
+
+def resync_step(g, o, scene, method="dfsph"):
+    """One step on both from the GPU's current state, the oracle forced to the GPU's iteration
+    counts (several counts are valid when err ~ eta: reading R20).  Returns (errors, gpu stats)."""
+    sync_oracle_to_gpu(g, o, scene)
+    if method == "dfsph":
+        g.sph_step_dfsph(1)
+        st = g.sph_read_stats()
+        fcg = st["cg_iters"] if scene.params["viscosity_mode"] == 2 else -1
+        fv = st["it_v"] if scene.params["enable_divergence_solve"] else -1
+        o.step_dfsph(forced_v=fv, forced_d=st["it_d"], forced_cg=fcg)
+    else:
+        g.sph_step_wcsph(1)
+        st = g.sph_read_stats()
+        o.step_wcsph()
+    return field_errors(g, o, scene), st

@@ -1,0 +1,372 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the fp64 oracle
+on the same seeded inputs.
+
+Bars (BASELINE.json north_star): cell offsets, cell keys and per-particle
+neighbour id sets BIT-EXACT; single-step density, alpha and velocity within 1e-4 in the norms of
+SURVEY.md 8(c.5): rho: max|d rho|/rho0; alpha: max|d alpha|/max|alpha|;
+v: max|dv| / max(max|v|, sqrt(|g| H)).  Positions follow from v: |dx| <= dt * tol * vscale + ulps.
+"""
+import numpy as np
+import pytest
+
+from paper_2403_11156_b200 import scenes
+
+from gpu_util import (assert_grid_parity, field_errors, make_pair, np_, resync_step, rows_to_sets,
+                      sync_oracle_to_gpu)
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4   # north_star: single-step density, alpha and velocity relative error <= 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2403_11156_b200 import binding, build
+    build.build()
+    binding.load()
+    return binding
+
+
+def check_errors(e, scene, tol=TOL):
+    assert e["rho"] <= tol, e
+    assert e["alpha"] <= tol, e
+    assert e["vel"] <= tol, e
+    dt = scene.params["dt"]
+    assert e["pos_abs"] <= dt * tol * e["vscale"] + 1e-6, e
+
+
+# ------------------------------------------------------------------ A1-A3 + neighbour sets
+
+GRID_SCENES = {
+    "random": lambda: scenes.random_cloud(3000, (0.4, 0.3, 0.2), seed=1, n_boundary=800),
+    "random_dense_ragged": lambda: scenes.random_cloud(4099, (0.33, 0.21, 0.17), seed=2, n_boundary=0),
+    "lattice": lambda: scenes.free_block((13, 11, 9)),
+    "jittered": lambda: scenes.free_block((17, 9, 12), jitter=0.2, seed=3),
+    "config0": lambda: scenes.config(0),
+    "splash_small": lambda: scenes.splash(n_target=3e4),
+}
+
+
+@pytest.mark.parametrize("name", list(GRID_SCENES))
+def test_grid_and_neighbor_sets_bit_exact(B, oracle, name):
+    sc = GRID_SCENES[name]()
+    g, o = make_pair(sc, oracle, max_fluid_neighbors=160, max_boundary_neighbors=96)
+    st = assert_grid_parity(g, o)
+    assert st["oob_count"] == 0
+    g.close(); o.close()
+
+
+def test_one_cell_and_cell_faces(B, oracle):
+    """Degenerate inputs: every particle in one cell; particles exactly on cell faces."""
+    rng = np.random.default_rng(5)
+    h = 0.04
+    sc = scenes.random_cloud(600, (0.9 * h, 0.9 * h, 0.9 * h), seed=7)
+    g, o = make_pair(sc, oracle, max_fluid_neighbors=640)
+    assert_grid_parity(g, o)
+    g.close(); o.close()
+    sc = scenes.random_cloud(1500, (0.3, 0.3, 0.3), seed=8)
+    c = np.float32(h) * np.float32(1.0009765625)
+    lo = np.asarray(sc.params["domain_min"], dtype=np.float32)
+    # snap a third of the coordinates onto multiples of the cell edge (fp32)
+    p = sc.fluid_pos.copy()
+    snap = rng.random(p.shape) < 0.33
+    p[snap] = (lo + np.round((p - lo) / c).astype(np.float32) * c)[snap]
+    sc.fluid_pos = p.astype(np.float32)
+    g, o = make_pair(sc, oracle, max_fluid_neighbors=160)
+    assert_grid_parity(g, o)
+    g.close(); o.close()
+
+
+def test_out_of_domain_clamped_and_counted(B, oracle):
+    sc = scenes.free_block((6, 6, 6))
+    p = sc.fluid_pos.copy()
+    p[0] += 10.0
+    p[1] -= 10.0
+    p[2, 2] += 5.0
+    sc.fluid_pos = p
+    g, o = make_pair(sc, oracle)
+    g.sph_build_grid(); o.build_grid()
+    assert g.sph_read_stats()["oob_count"] == o.stats()["oob_count"] == 3
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_OF_PARTICLE)), o.cell_of_particle(0))
+    g.close(); o.close()
+
+
+def test_neighbor_list_overflow_is_flagged(B, oracle):
+    sc = scenes.free_block((8, 8, 8))
+    g, o = make_pair(sc, oracle, max_fluid_neighbors=16)
+    g.sph_build_grid()
+    st = g.sph_read_stats()
+    assert st["overflow_count"] > 0 and st["max_fluid_neighbors"] > 16
+    g.close(); o.close()
+
+
+def test_empty_and_tiny_inputs(B, oracle):
+    # one particle, no boundary
+    sc = scenes.free_block((1, 1, 1), gravity=(0.0, 0.0, -9.81))
+    g, o = make_pair(sc, oracle)
+    g.sph_step_dfsph(3)
+    v = np_(g.sph_read_state(B.VEL))
+    assert np.allclose(v[0], [0, 0, -9.81 * 3 * sc.params["dt"]], rtol=1e-6)
+    assert g.sph_read_stats()["steps_done"] == 3
+    g.close(); o.close()
+    # no fluid at all, only boundary
+    sc = scenes.config(0)
+    sc.fluid_pos = sc.fluid_pos[:0]; sc.fluid_vel = sc.fluid_vel[:0]
+    g = B.Sim.from_scene(sc)
+    g.sph_step_dfsph(2)
+    assert g.sph_read_stats()["steps_done"] == 2
+    assert np_(g.sph_read_state(B.POS)).shape == (0, 3)
+    g.close()
+
+
+# ------------------------------------------------------------------ A4, A8 static fields
+
+def test_density_alpha_psi_parity(B, oracle):
+    for sc in (scenes.config(0), scenes.splash(n_target=3e4), scenes.free_block((12, 12, 12), jitter=0.15, seed=4)):
+        g, o = make_pair(sc, oracle)
+        g.sph_build_grid(); o.build_grid(); o.compute_density_alpha()
+        rho0 = sc.params["rest_density"]
+        rho = np_(g.sph_read_state(B.DENSITY)).astype(np.float64)
+        al = np_(g.sph_read_state(B.ALPHA)).astype(np.float64)
+        assert np.abs(rho - o.density()).max() / rho0 <= 1e-5
+        assert np.abs(al - o.alpha()).max() / np.abs(o.alpha()).max() <= 1e-5
+        if g.nb:
+            psi = np_(g.sph_read_state(B.BOUNDARY_PSI)).astype(np.float64)
+            assert np.abs(psi - o.psi()).max() / np.abs(o.psi()).max() <= 1e-5
+        g.close(); o.close()
+
+
+# ------------------------------------------------------------------ whole steps, resync protocol
+
+def run_resync(B, oracle, sc, n_steps, checkpoints, method="dfsph", tol=TOL, **over):
+    g, o = make_pair(sc, oracle, **over)
+    worst = {}
+    done = 0
+    hist = []
+    for cp in checkpoints:
+        while done < cp:
+            (g.sph_step_dfsph if method == "dfsph" else g.sph_step_wcsph)(1)
+            done += 1
+        e, st = resync_step(g, o, sc, method)
+        done += 1
+        hist.append((cp, e, st))
+        check_errors(e, sc, tol)
+        assert st["overflow_count"] == 0 and st["nan_count"] == 0 and st["oob_count"] == 0, st
+        for k, v in e.items():
+            worst[k] = max(worst.get(k, 0.0), v)
+    while done < n_steps:
+        (g.sph_step_dfsph if method == "dfsph" else g.sph_step_wcsph)(1)
+        done += 1
+    st = g.sph_read_stats()
+    assert st["steps_done"] == n_steps
+    return g, o, worst, hist
+
+
+def test_config0_dfsph_step_parity(B, oracle):
+    """BASELINE config 0 (8,000 particles, 100 steps): resync parity at steps 0, 1, 10, 50, 99;
+    DFSPH exits every checked step with average density error < 0.1 %."""
+    sc = scenes.config(0)
+    g, o, worst, hist = run_resync(B, oracle, sc, 100, [0, 1, 10, 50, 99])
+    for cp, e, st in hist:
+        assert st["err_rho"] < 1e-3, (cp, st)
+        assert st["it_d"] >= 2 and st["it_v"] >= 1
+    # free-running oracle from the same state picks the same iteration counts (+-1)
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_step_dfsph(1)
+    o.step_dfsph()
+    st, so = g.sph_read_stats(), o.stats()
+    assert abs(st["it_v"] - so["it_v"]) <= 1 and abs(st["it_d"] - so["it_d"]) <= 1
+    assert abs(st["err_rho"] - so["err_rho"]) <= 1e-6 and abs(st["err_v"] - so["err_v"]) <= 1e-6
+    g.close(); o.close()
+
+
+def test_config1_scaled_explicit_viscosity_and_wcsph(B, oracle):
+    """Config 1 at reduced size (24^3 block, Eq. 15 viscosity 0.01): DFSPH and WCSPH steps."""
+    kw = dict(viscosity_mode=1, kinematic_viscosity=0.01)
+    sc = scenes.dam_break((24, 24, 24), (48, 24, 24), steps=30, **kw)
+    g, o, worst, _ = run_resync(B, oracle, sc, 30, [0, 5, 29])
+    g.close(); o.close()
+    scw = scenes.dam_break((24, 24, 24), (48, 24, 24), dt=1e-4, steps=40, **kw)
+    g, o, worst, _ = run_resync(B, oracle, scw, 40, [0, 10, 39], method="wcsph")
+    g.close(); o.close()
+
+
+def test_config2_scaled_rigid_coupling(B, oracle):
+    """Config 2 at half scale: three dynamic bodies; Eq. 14 reactions and body states."""
+    sc = scenes.rigid_coupling(scale=0.5, seed=0, steps=12)
+    g, o = make_pair(sc, oracle)
+    # let the fluid reach the bodies quickly: give it a downward velocity
+    import torch
+    v0 = torch.zeros((g.nf, 3), dtype=torch.float32, device="cuda"); v0[:, 2] = -3.0
+    g.sph_write_state(B.VEL, v0)
+    # move the block down so that it touches the bodies within a few steps
+    p0 = g.sph_read_state(B.POS).clone(); p0[:, 2] -= 0.18
+    g.sph_write_state(B.POS, p0)
+    worst_f = 0.0
+    for k in range(12):
+        e, st = resync_step(g, o, sc)
+        check_errors(e, sc)
+        fg = np_(g.sph_read_state(B.BOUNDARY_FORCE)).astype(np.float64)
+        fo = o.boundary_force()
+        fscale = max(np.abs(fo).max(), 1e-12)
+        worst_f = max(worst_f, np.abs(fg - fo).max() / fscale)
+        if np.abs(fo).max() > 0:
+            assert np.abs(fg - fo).max() <= 2e-4 * fscale + 1e-9
+        for bg, bo in zip(g.read_bodies(), o.bodies()):
+            for key in ("com", "lin_vel", "ang_vel", "quat"):
+                assert np.allclose(np.asarray(bg[key], dtype=np.float64), bo[key], rtol=1e-4, atol=2e-6), (k, key, bg[key], bo[key])
+        bp = np_(g.sph_read_state(B.BOUNDARY_POS)).astype(np.float64)
+        assert np.abs(bp - o.boundary_pos()).max() <= 2e-6
+    assert np.abs(o.boundary_force()).max() > 0, "the test must exercise the coupling"
+    g.close(); o.close()
+
+
+def test_config3_scaled_implicit_viscosity(B, oracle):
+    """Config 3 at 0.3 scale: matrix-free CG (Eq. 16-19), nu = 10, tol 1e-5."""
+    sc = scenes.viscous_column(scale=0.3, steps=8)
+    g, o = make_pair(sc, oracle)
+    for k in range(6):
+        e, st = resync_step(g, o, sc)
+        check_errors(e, sc)
+        so = o.stats()
+        assert st["cg_iters"] == so["cg_iters"] > 0
+        assert abs(st["cg_residual"] - so["cg_residual"]) <= 1e-3 * max(so["cg_residual"], 1e-7) + 2e-6
+    # free-running oracle: iteration count close to the GPU's
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_step_dfsph(1); o.step_dfsph()
+    st, so = g.sph_read_stats(), o.stats()
+    assert abs(st["cg_iters"] - so["cg_iters"]) <= 2
+    assert st["cg_residual"] <= 1.5e-5
+    g.close(); o.close()
+
+
+def test_config4_scaled_splash(B, oracle):
+    sc = scenes.splash(n_target=4e4, steps=40)
+    g, o, worst, hist = run_resync(B, oracle, sc, 40, [0, 1, 20, 39])
+    for cp, e, st in hist:
+        assert st["err_rho"] < 1e-3
+    g.close(); o.close()
+
+
+# ------------------------------------------------------------------ modes of the library
+
+def test_bitwise_determinism_and_mode_equivalence(B, oracle):
+    """Same input twice -> bit-identical state (R12); CUDA-graph WHILE loops == host-driven loops;
+    neighbour-list passes == 27-cell-walk passes (same summation order) bit for bit."""
+    sc = scenes.splash(n_target=2e4)
+    outs = []
+    for over in (dict(), dict(), dict(use_cuda_graph=0), dict(use_neighbor_list=0)):
+        g = B.Sim.from_scene(sc, **over)
+        g.sph_step_dfsph(15)
+        outs.append((np_(g.sph_read_state(B.POS)), np_(g.sph_read_state(B.VEL)), g.sph_read_stats()))
+        g.close()
+    for p, v, st in outs[1:]:
+        assert np.array_equal(p, outs[0][0]) and np.array_equal(v, outs[0][1])
+        assert st["total_it_d"] == outs[0][2]["total_it_d"] and st["total_it_v"] == outs[0][2]["total_it_v"]
+
+
+def test_forced_iterations_and_solver_loop_semantics(B, oracle):
+    """sph_set_forced_iterations: exact counts without re-capturing the graph; forced 0 skips."""
+    sc = scenes.config(0)
+    g, o = make_pair(sc, oracle)
+    g.sph_set_forced_iterations(3, 5, -1)
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_step_dfsph(1)
+    st = g.sph_read_stats()
+    assert (st["it_v"], st["it_d"]) == (3, 5)
+    o.step_dfsph(forced_v=3, forced_d=5)
+    check_errors(field_errors(g, o, sc), sc)
+    g.sph_set_forced_iterations(0, 0, -1)
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_step_dfsph(1)
+    st = g.sph_read_stats()
+    assert (st["it_v"], st["it_d"]) == (0, 0)
+    o.step_dfsph(forced_v=0, forced_d=0)
+    check_errors(field_errors(g, o, sc), sc)
+    g.sph_set_forced_iterations(-1, -1, -1)
+    g.sph_step_dfsph(1)
+    st = g.sph_read_stats()
+    assert st["it_v"] >= 1 and st["it_d"] >= 2
+    assert g.sph_launch_count() > 0
+    g.close(); o.close()
+
+
+def test_state_roundtrip_host_and_device(B, oracle):
+    """sph_write_state / sph_read_state through device and host buffers (the e2e path of bench.py)."""
+    import torch
+    sc = scenes.config(0)
+    g = B.Sim.from_scene(sc)
+    g.sph_step_dfsph(3)
+    p = g.sph_read_state(B.POS).clone(); v = g.sph_read_state(B.VEL).clone()
+    ph = torch.empty((g.nf, 3), dtype=torch.float32).pin_memory()
+    vh = torch.empty((g.nf, 3), dtype=torch.float32).pin_memory()
+    g.sph_read_state_host(B.POS, ph); g.sph_read_state_host(B.VEL, vh)
+    assert torch.equal(ph, p.cpu()) and torch.equal(vh, v.cpu())
+    g2 = B.Sim.from_scene(sc)
+    g2.sph_write_state(B.POS, ph); g2.sph_write_state(B.VEL, vh)
+    with pytest.raises(B.SphError):
+        g2.sph_read_state(B.DENSITY)          # stale until the next grid build
+    g.sph_step_dfsph(2); g2.sph_step_dfsph(2)
+    assert torch.equal(g.sph_read_state(B.POS), g2.sph_read_state(B.POS))
+    assert torch.equal(g.sph_read_state(B.VEL), g2.sph_read_state(B.VEL))
+    g.close(); g2.close()
+
+
+# ------------------------------------------------------------------ full size, bench configuration
+
+def test_config4_full_size_sampled_parity(B, oracle):
+    """BASELINE config 4 (1.23M fluid particles), in the configuration bench.py times (CUDA graph,
+    neighbour lists): cell offsets bit-exact; on a seeded sample of particles the neighbour sets
+    (by brute force over ALL particles with the fp32 predicate of R10, independent of any grid)
+    bit-exact and density / alpha vs the oracle within 1e-4; after 5 steps, invariants."""
+    sc = scenes.config(4)
+    g = B.Sim.from_scene(sc)
+    o = oracle.Sim.from_scene(sc)
+    g.sph_build_grid()
+    o.build_grid(); o.compute_density_alpha()
+    st = g.sph_read_stats()
+    assert st["overflow_count"] == 0 and st["oob_count"] == 0
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_OF_PARTICLE)), o.cell_of_particle(0))
+    rng = np.random.default_rng(0)
+    sample = rng.choice(g.nf, size=300, replace=False)
+    # include particles next to walls / obstacles: those with boundary neighbours
+    cnt = np_(g.sph_read_state(B.NEIGHBOR_COUNT))
+    near = np.nonzero(cnt[:, 1] > 0)[0]
+    sample = np.concatenate([sample, rng.choice(near, size=200, replace=False)])
+    rows_f = np_(g.sph_read_state(B.FLUID_NEIGHBORS)[torch_index(sample)])
+    rows_b = np_(g.sph_read_state(B.BOUNDARY_NEIGHBORS)[torch_index(sample)])
+    h2 = np.float32(sc.params["support_radius"]) * np.float32(sc.params["support_radius"])
+    fp, bp = sc.fluid_pos, sc.boundary_pos
+    for r, i in enumerate(sample):
+        for pts, rows, skip in ((fp, rows_f, i), (bp, rows_b, -1)):
+            d = (fp[i][None, :] - pts).astype(np.float32)
+            d64 = d.astype(np.float64)
+            t = (d64[:, 0] * d64[:, 0]).astype(np.float32).astype(np.float64)
+            t = (d64[:, 1] * d64[:, 1] + t).astype(np.float32).astype(np.float64)
+            d2 = (d64[:, 2] * d64[:, 2] + t).astype(np.float32)
+            ids = set(np.nonzero(d2 < h2)[0].tolist()) - {skip}
+            assert ids == set(int(v) for v in rows[r][rows[r] >= 0]), (i, skip)
+    rho = np_(g.sph_read_state(B.DENSITY)).astype(np.float64)
+    al = np_(g.sph_read_state(B.ALPHA)).astype(np.float64)
+    assert np.abs(rho - o.density()).max() / 1000.0 <= TOL
+    assert np.abs(al - o.alpha()).max() / np.abs(o.alpha()).max() <= TOL
+    o.close()
+    g.sph_step_dfsph(5)
+    st = g.sph_read_stats()
+    assert st["steps_done"] == 5 and st["nan_count"] == 0 and st["overflow_count"] == 0
+    assert st["err_rho"] < 1e-3 and 1.9 < st["v_max"] < 4.0
+    p = np_(g.sph_read_state(B.POS))
+    assert np.isfinite(p).all()
+    lo, hi = np.asarray(sc.params["tank_min"]), np.asarray(sc.params["tank_max"])
+    assert (p > lo - 0.02).all() and (p < hi + 0.02).all()
+    g.close()
+
+
+def torch_index(a):
+    import torch
+    return torch.as_tensor(np.asarray(a), dtype=torch.long, device="cuda")
