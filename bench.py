@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py -- DFSPH particle-steps/s on BASELINE.json's headline workload (config 4: 1.23M fluid
+particles, two blocks colliding against four static obstacles in a 4x2x2 m tank), one B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: grid build, density +
+alpha + neighbour lists, divergence-free solve, gravity, constant-density solve, integration.
+Prints ONE JSON line (rank 0).  N > 1: independent replicas, one per GPU (the path has no
+exchange step in this version: DESIGN.md section 8), reported as weak scaling.
+
+--impl reference times the fp64 CPU oracle (oracle/), as it stands, on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "DFSPH particle-steps/sec at 1.23M particles (1 B200); achieved HBM GB/s vs peak"
+UNIT = "particle-steps/s"
+FP32_LANES_PER_SM = 128
+N_SM = 148
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); smax.append(float(r[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, r[5:9]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return dict(sm_mhz=(sm[len(sm) // 2] if sm else None), sm_max_mhz=(max(smax) if smax else None),
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+# ---------------------------------------------------------------------------------------------
+# Algorithmic work per fluid particle of each kernel:
+# compulsory bytes = own inputs read once + outputs written once, neighbour gathers assumed
+# cache-served; nf / nbd = mean fluid / boundary neighbours, cand = mean candidates of the 27-cell walk.
+def kernel_work(name, nf_mean, nb_mean, cand_mean):
+    lst = 4.0 * (nf_mean + nb_mean)
+    if name == "k_density_alpha":      # A4 + list build: pos in; rho, alpha, count, list out
+        return dict(bytes=16 + 4 + 4 + 4 + lst, flops=8.0 * cand_mean + 34.0 * (nf_mean + nb_mean) + 25, row="A4")
+    if name == "k_solver_p":           # pos, vel, alpha, count, list in; posk out
+        return dict(bytes=16 + 16 + 4 + 4 + lst + 16, flops=27.0 * (nf_mean + nb_mean) + 12, row="A5/A7 P")
+    if name == "k_solver_c":           # posk, count, list, vel in; vel out
+        return dict(bytes=16 + 4 + lst + 16 + 16, flops=26.0 * (nf_mean + nb_mean) + 12, row="A5/A7 C")
+    if name == "k_reorder":            # slot, key, cell range, pos, vel, id in; pos, vel, id out
+        return dict(bytes=4 + 4 + 8 + 36 + 36, flops=0.0, row="A3")
+    if name == "k_cell_key_hist":
+        return dict(bytes=16 + 4 + 4 + 8, flops=10.0, row="A1")
+    if name == "k_integrate":
+        return dict(bytes=36 + 36, flops=12.0, row="A9")
+    if name == "k_gravity":
+        return dict(bytes=32, flops=6.0, row="A6")
+    return None
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    from paper_2403_11156_b200 import binding as B, build, scenes
+    build.build()
+    B.load()
+    peaks = load_peaks()
+
+    sc = scenes.config(args.config, seed=rank)
+    K, W = args.steps, args.warmup
+    sim = B.Sim.from_scene(sc, device=local_rank, use_cuda_graph=0 if args.no_graph else 1)
+    stream = sim.stream
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
+    sim.sph_step_dfsph(W)
+    launches0 = sim.sph_launch_count()
+    st0 = sim.sph_read_stats()
+    clocks = ClockSampler(local_rank)
+    barrier()
+    clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sim.sph_step_dfsph(K)
+    e1.record(stream)
+    stream.synchronize()
+    barrier()
+    ck = clocks.stop()
+    ms = e0.elapsed_time(e1)
+    st1 = sim.sph_read_stats()
+    launches = sim.sph_launch_count() - launches0
+    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    ms_max = float(tms.item())
+    nf = sc.n_fluid
+    value = world * nf * K / (ms_max * 1e-3)
+    mean_it_v = (st1["total_it_v"] - st0["total_it_v"]) / max(K, 1)
+    mean_it_d = (st1["total_it_d"] - st0["total_it_d"]) / max(K, 1)
+
+    # ---- end to end through the C ABI with HOST buffers: every step uploads positions and
+    # velocities from pinned host memory and reads the new ones back
+    Ke = max(1, min(K, args.e2e_steps))
+    ph = torch.empty((nf, 3), dtype=torch.float32).pin_memory()
+    vh = torch.empty((nf, 3), dtype=torch.float32).pin_memory()
+    sim.sph_read_state_host(B.POS, ph); sim.sph_read_state_host(B.VEL, vh)
+    for _ in range(3):
+        sim.sph_write_state(B.POS, ph); sim.sph_write_state(B.VEL, vh)
+        sim.sph_step_dfsph(1)
+        sim.sph_read_state_host(B.POS, ph); sim.sph_read_state_host(B.VEL, vh)
+    barrier()
+    e0.record(stream)
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        sim.sph_write_state(B.POS, ph); sim.sph_write_state(B.VEL, vh)
+        sim.sph_step_dfsph(1)
+        sim.sph_read_state_host(B.POS, ph); sim.sph_read_state_host(B.VEL, vh)
+    e1.record(stream)
+    stream.synchronize()
+    wall = time.perf_counter() - t0
+    barrier()
+    ems = max(e0.elapsed_time(e1), wall * 1e3)
+    tms = torch.tensor([ems], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+    e2e_value = world * nf * Ke / (float(tms.item()) * 1e-3)
+    sim.close()
+
+    out = None
+    if rank == 0:
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": sc.name, "n_fluid": nf, "n_boundary": sc.n_boundary,
+                       "n_cells": int(sim.ncells), "dt": sc.params["dt"], "solver": "DFSPH",
+                       "mean_it_v": mean_it_v, "mean_it_d": mean_it_d,
+                       "neighbour_passes_per_step": 1 + 2 * mean_it_v + 2 * mean_it_d,
+                       "parallelism": "replicas x%d" % world if world > 1 else "1 GPU",
+                       "launch_mode": "host-driven launches (--no-graph)" if args.no_graph else "one CUDA graph per step, device-side WHILE loops",
+                       "l2": "no flush: the per-step working set (lists + SoA store, ~%d MB) exceeds the 126 MB L2"
+                             % int(sim.workspace_bytes / 2 ** 20 * 0.6),
+                       "err_rho_last": st1["err_rho"], "v_max_last": st1["v_max"]},
+            "clocks": ck,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nf * 24, "d2h_bytes_per_step": nf * 24,
+                    "steps": Ke},
+            "gpu_launches": int(launches),
+        }
+
+    # ---- per-kernel CUDA-event timing over the same W + K steps (host-driven launch mode: events
+    # cannot bracket nodes inside a graph's WHILE body), rank 0 only -> roofline of the dominant kernel
+    if rank == 0 and not args.no_breakdown:
+        sim2 = B.Sim.from_scene(sc, device=local_rank, use_cuda_graph=0)
+        sim2.sph_step_dfsph(W)
+        sim2.sph_build_grid()   # no-op for the physics: refreshes lists for the statistics below
+        cnt = sim2.sph_read_state(B.NEIGHBOR_COUNT).to(torch.float64)
+        nf_mean, nb_mean = float(cnt[:, 0].mean()), float(cnt[:, 1].mean())
+        cs = sim2.sph_read_state(B.CELL_START).to(torch.int64)
+        occ = (cs[1:] - cs[:-1]).to(torch.float32).reshape(1, 1, sim2.nz, sim2.ny, sim2.nx)
+        # candidates per particle of the 27-cell walk = occupancy of the 3x3x3 cell box around it
+        box = 27.0 * torch.nn.functional.avg_pool3d(occ, 3, stride=1, padding=1, count_include_pad=True)
+        cand_mean = float((occ * box).sum() / max(float(occ.sum()), 1.0))
+        sim2.sph_enable_kernel_timing(True)
+        sim2.sph_step_dfsph(K)
+        kt = sim2.sph_read_kernel_times()
+        sim2.close()
+        tot = sum(v[1] for v in kt.values())
+        table = {k: {"launches": v[0], "ms_total": round(v[1], 3), "us_avg": round(1e3 * v[1] / v[0], 2),
+                     "share": round(v[1] / tot, 4)} for k, v in sorted(kt.items(), key=lambda kv: -kv[1][1])}
+        top = next(iter(table))
+        work = kernel_work(top, nf_mean, nb_mean, cand_mean)
+        dur = 1e-3 * kt[top][1] / kt[top][0]
+        fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        roof = {"kernel": top, "row": work["row"] if work else None, "avg_us": round(dur * 1e6, 2),
+                "share_of_step": table[top]["share"], "traffic": None,
+                "peak_source": peaks["source"] + " (MEASURED_PEAKS.json)"}
+        if work:
+            gbs = work["bytes"] * nf / dur / 1e9
+            tfl = work["flops"] * nf / dur / 1e12
+            if top == "k_density_alpha":
+                roof.update({"bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s",
+                             "frac": tfl / fp32_peak, "hbm_achieved_gbs": gbs, "hbm_frac": gbs / peaks["hbm_gbs"]})
+            else:
+                roof.update({"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                             "frac": gbs / peaks["hbm_gbs"], "alu_achieved_tflops": tfl, "alu_frac": tfl / fp32_peak})
+        per_kernel = {}
+        for k in table:
+            w = kernel_work(k, nf_mean, nb_mean, cand_mean)
+            if w:
+                d = 1e-3 * kt[k][1] / kt[k][0]
+                per_kernel[k] = {"row": w["row"], "us_avg": table[k]["us_avg"], "share": table[k]["share"],
+                                 "hbm_gbs": round(w["bytes"] * nf / d / 1e9, 1),
+                                 "hbm_frac": round(w["bytes"] * nf / d / 1e9 / peaks["hbm_gbs"], 4),
+                                 "fp32_tflops": round(w["flops"] * nf / d / 1e12, 2)}
+        out["roofline"] = roof
+        out["kernels"] = per_kernel
+        out["kernel_time_table"] = table
+        out["config"].update({"mean_fluid_neighbours": nf_mean, "mean_boundary_neighbours": nb_mean,
+                              "mean_candidates": cand_mean,
+                              "kernel_ms_per_step_sum": tot / K})
+
+    # ---- the oracle on the host cores, bounded sample (rank 0, N = 1 only)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = time_oracle(sc, budget_s=args.cpu_budget)
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def time_oracle(sc, budget_s=20.0, steps=None):
+    """Oracle (as it stands) on this box's host cores: DFSPH steps of the same scene from its
+    initial state, as many as fit the budget (at least 2)."""
+    from oracle import sphref
+    sphref.build()
+    o = sphref.Sim.from_scene(sc)
+    t0 = time.perf_counter()
+    o.step_dfsph()
+    t1 = time.perf_counter() - t0
+    n = steps if steps is not None else max(2, min(50, int(budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    for _ in range(n):
+        o.step_dfsph()
+    dt = time.perf_counter() - t0
+    so = o.stats()
+    o.close()
+    return {"value": sc.n_fluid * n / dt, "unit": UNIT, "cores": sphref.num_threads(), "kind": "oracle",
+            "sample": "%d DFSPH steps of %s (%d fluid particles) after 1 untimed step; it_v=%d it_d=%d in the last"
+                      % (n, sc.name, sc.n_fluid, so["it_v"], so["it_d"]),
+            "s_per_step": dt / n}
+
+
+def run_reference(args):
+    """Reference arm = the fp64 oracle on the host cores (there is no other reference
+    implementation: /root/reference holds only the paper).  Each step is one oracle DFSPH step on
+    a bounded sample of the workload: the config-4 scene generator at a particle count chosen so
+    that W + K steps end within ~2 minutes."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    from paper_2403_11156_b200 import scenes
+    from oracle import sphref
+    sphref.build()
+    K, W = args.steps, args.warmup
+    full = scenes.config(args.config, seed=0)
+    o = sphref.Sim.from_scene(full)
+    t0 = time.perf_counter(); o.step_dfsph(); t_full = time.perf_counter() - t0
+    o.close()
+    budget = 120.0
+    frac = min(1.0, budget / max((K + W) * t_full, 1e-9))
+    if frac >= 1.0 or args.config != 4:
+        sc = full
+    else:
+        sc = scenes.splash(n_target=max(2e4, 1.23e6 * frac), seed=0, name="config4_splash_sample")
+    o = sphref.Sim.from_scene(sc)
+    for _ in range(W):
+        o.step_dfsph()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        o.step_dfsph()
+    dt = time.perf_counter() - t0
+    o.close()
+    value = sc.n_fluid * K / dt
+    sample = "%d oracle DFSPH steps on the config-4 scene generator at %d fluid particles (%.1f%% of 1.23M)" % (
+        K, sc.n_fluid, 100.0 * sc.n_fluid / 1.23e6)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": W, "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": full.name, "sample_n_fluid": sc.n_fluid, "solver": "DFSPH"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": sphref.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--e2e-steps", type=int, default=50)
+    ap.add_argument("--cpu-budget", type=float, default=20.0)
+    ap.add_argument("--no-graph", action="store_true",
+                    help="host-driven launches instead of the CUDA graph (ncu cannot profile kernel nodes of a "
+                         "graph that has conditional nodes): for profiling commands only")
+    ap.add_argument("--no-breakdown", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -199,6 +199,14 @@ int sph_read_stats(SphSim *sim, SphStats *dst_host);
  * loop bodies once per executed iteration) issued for this simulation since create. */
 long long sph_launch_count(SphSim *sim);
 
+/* Per-kernel timing for roofline reports: with SphParams.use_cuda_graph == 0, every kernel
+ * launch of the following steps is bracketed by a pair of CUDA events on the simulation's stream.
+ * sph_read_kernel_times synchronises, then writes one text line per kernel,
+ * "<kernel name> <launches> <total milliseconds>\n", NUL-terminated, into buf (SPH_ENOMEM if it
+ * does not fit) and clears the record. */
+int sph_enable_kernel_timing(SphSim *sim, int enable);
+int sph_read_kernel_times(SphSim *sim, char *buf, size_t bytes);
+
 const char *sph_last_error(const SphSim *sim);
 void sph_destroy(SphSim *sim);
 

@@ -25,7 +25,8 @@ SPH_OK, SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA, SPH_EDOMAIN, SPH_ESTATE = 0, -1, -2, 
 
 EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid", "sph_step_dfsph",
            "sph_step_wcsph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
-           "sph_read_stats", "sph_launch_count", "sph_last_error", "sph_destroy"]
+           "sph_read_stats", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
+           "sph_last_error", "sph_destroy"]
 
 
 class SphParams(C.Structure):
@@ -107,6 +108,8 @@ def load() -> C.CDLL:
         L.sph_read_stats.argtypes = [C.c_void_p, C.POINTER(SphStats)]
         L.sph_launch_count.restype = C.c_longlong
         L.sph_launch_count.argtypes = [C.c_void_p]
+        L.sph_enable_kernel_timing.argtypes = [C.c_void_p, C.c_int]
+        L.sph_read_kernel_times.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
         L.sph_last_error.restype = C.c_char_p
         L.sph_last_error.argtypes = [C.c_void_p]
         L.sph_destroy.argtypes = [C.c_void_p]
@@ -309,6 +312,19 @@ class Sim:
         s = SphStats()
         self._check(load().sph_read_stats(self._h, C.byref(s)))
         return {k: getattr(s, k) for k, _ in SphStats._fields_}
+
+    def sph_enable_kernel_timing(self, enable: bool = True):
+        self._check(load().sph_enable_kernel_timing(self._h, int(enable)))
+
+    def sph_read_kernel_times(self) -> Dict[str, tuple]:
+        """{kernel name: (launches, total ms)} since the last call."""
+        buf = C.create_string_buffer(1 << 16)
+        self._check(load().sph_read_kernel_times(self._h, buf, len(buf)))
+        out = {}
+        for line in buf.value.decode().splitlines():
+            name, n, ms = line.split()
+            out[name] = (int(n), float(ms))
+        return out
 
     def sph_launch_count(self) -> int:
         return int(load().sph_launch_count(self._h))

@@ -77,6 +77,11 @@ struct SphSim {
     long long graph_steps[2] = { 0, 0 };              // graph launches per method (host view)
     long long misc_launches = 0;
     long long *cur_counter = nullptr;
+    // optional per-kernel CUDA-event timing (host-driven launch mode only, see sph_enable_kernel_timing)
+    bool timing = false;
+    struct TimedLaunch { const char *name; cudaEvent_t a, b; };
+    std::vector<TimedLaunch> timed;
+    std::vector<cudaEvent_t> event_pool;
     std::string err;
 };
 
@@ -95,10 +100,27 @@ namespace {
 
 #define LAUNCH(sim, kern, grid, block, strm, ...)                                               \
     do {                                                                                        \
+        cudaEvent_t ea_ = nullptr, eb_ = nullptr;                                               \
+        if ((sim)->timing) {                                                                    \
+            ea_ = take_event(sim); eb_ = take_event(sim);                                       \
+            cudaEventRecord(ea_, (strm));                                                       \
+        }                                                                                       \
         kern<<<(grid), (block), 0, (strm)>>>(__VA_ARGS__);                                      \
+        if ((sim)->timing) {                                                                    \
+            cudaEventRecord(eb_, (strm));                                                       \
+            (sim)->timed.push_back({ #kern, ea_, eb_ });                                        \
+        }                                                                                       \
         ++*(sim)->cur_counter;                                                                  \
         CUDA_TRY(sim, cudaGetLastError());                                                      \
     } while (0)
+
+inline cudaEvent_t take_event(SphSim *s)
+{
+    cudaEvent_t e = nullptr;
+    if (!s->event_pool.empty()) { e = s->event_pool.back(); s->event_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
@@ -372,7 +394,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
             if (rc) return rc;
             // non-pressure accelerations (A6 / A11)
             if (s->prm.viscosity_mode == 1) {
-                LAUNCH(s, k_explicit_viscosity<LIST>, s->nblocks, kBlock, st, p, s->velB, s->velC);
+                LAUNCH(s, (k_explicit_viscosity<LIST, false>), s->nblocks, kBlock, st, p, s->velB, s->velC);
                 vcur = s->velC;
             } else {
                 LAUNCH(s, k_gravity, cdiv(nf, 256), 256, st, s->c, s->velB, s->velB);
@@ -403,7 +425,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
             // WCSPH (A10)
             LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->velB, s->posk);
             if (s->prm.viscosity_mode == 1) {
-                LAUNCH(s, k_explicit_viscosity<LIST>, s->nblocks, kBlock, st, p, s->velB, s->velC);
+                LAUNCH(s, (k_explicit_viscosity<LIST, true>), s->nblocks, kBlock, st, p, s->velB, s->velC);
                 vcur = s->velC;
             } else {
                 LAUNCH(s, k_gravity, cdiv(nf, 256), 256, st, s->c, s->velB, s->velB);
@@ -794,6 +816,41 @@ long long sph_launch_count(SphSim *s)
     return n;
 }
 
+int sph_enable_kernel_timing(SphSim *s, int enable)
+{
+    if (!s) return SPH_EINVAL;
+    if (enable && s->prm.use_cuda_graph) { s->err = "kernel timing needs use_cuda_graph = 0 (events cannot bracket nodes of a loop body)"; return SPH_ESTATE; }
+    s->timing = enable != 0;
+    return SPH_OK;
+}
+
+int sph_read_kernel_times(SphSim *s, char *buf, size_t bytes)
+{
+    if (!s || !buf || bytes == 0) return SPH_EINVAL;
+    DeviceGuard dg(s->device);
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    struct Acc { std::string name; long long n; double ms; };
+    std::vector<Acc> acc;
+    for (auto &t : s->timed) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t.a, t.b);
+        std::string nm = t.name;
+        // strip template arguments, parentheses and the namespace
+        size_t lt = nm.find('<'); if (lt != std::string::npos) nm = nm.substr(0, lt);
+        while (!nm.empty() && (nm[0] == '(' || nm[0] == ' ')) nm.erase(0, 1);
+        bool found = false;
+        for (auto &a : acc) if (a.name == nm) { a.n++; a.ms += ms; found = true; break; }
+        if (!found) acc.push_back({ nm, 1, ms });
+        s->event_pool.push_back(t.a); s->event_pool.push_back(t.b);
+    }
+    s->timed.clear();
+    std::string out;
+    for (auto &a : acc) { char line[160]; snprintf(line, sizeof line, "%s %lld %.6f\n", a.name.c_str(), a.n, a.ms); out += line; }
+    if (out.size() + 1 > bytes) { s->err = "buffer too small"; return SPH_ENOMEM; }
+    memcpy(buf, out.c_str(), out.size() + 1);
+    return SPH_OK;
+}
+
 const char *sph_last_error(const SphSim *s) { return s ? s->err.c_str() : g_create_error.c_str(); }
 
 void sph_destroy(SphSim *s)
@@ -804,6 +861,8 @@ void sph_destroy(SphSim *s)
     for (int m = 0; m < 2; ++m) if (s->exec[m]) cudaGraphExecDestroy(s->exec[m]);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     if (s->pinned) cudaFreeHost(s->pinned);
+    for (auto &t : s->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
+    for (auto e : s->event_pool) cudaEventDestroy(e);
     delete s;
 }
 

@@ -276,8 +276,9 @@ k_gravity(SimConst c, const float4 *__restrict__ vin, float4 *__restrict__ vout)
 
 // mode 1: explicit viscosity, Eq. 15 (R4, R16, R22):
 //   a_i = nu 2(d+2) sum_j (m / rho_j) (v_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij, fluid-fluid only.
-// rho_j is vel[j].w (rho for DFSPH, the clamped rho~ for WCSPH).  Reads vin, writes vout != vin.
-template <bool LIST>
+// rho_j is vel[j].w; CLAMP = true (WCSPH, R17) uses rho~_j = max(rho_j, rho0).  Reads vin, writes
+// vout != vin.
+template <bool LIST, bool CLAMP>
 __global__ void __launch_bounds__(kBlock)
 k_explicit_viscosity(PassCtx p, const float4 *__restrict__ vin, float4 *__restrict__ vout)
 {
@@ -291,7 +292,8 @@ k_explicit_viscosity(PassCtx p, const float4 *__restrict__ vin, float4 *__restri
         [&](int j, float4, float dx, float dy, float dz, float d2) {
             float4 vj = __ldg(vin + j);
             float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
-            float s = pair_gradf(c, d2) * dv / ((d2 + c.visc_eps) * vj.w);
+            float rj = CLAMP ? fmaxf(vj.w, c.rho0) : vj.w;
+            float s = pair_gradf(c, d2) * dv / ((d2 + c.visc_eps) * rj);
             ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay); az = fmaf(s, dz, az);
         },
         [&](int, float4, float, float, float, float) {});
@@ -389,9 +391,9 @@ k_cg_direction(int n, const DevControl *__restrict__ ctl, const float4 *__restri
 // ---------------------------------------------------------------------------------------------
 // A10: WCSPH equation of state (R17): rho~ = max(rho, rho0),
 // p = k((rho~/rho0)^gamma - 1), evaluated as k expm1(gamma log1p(delta)), delta = (rho~ - rho0)/rho0,
-// which keeps the small excess accurate in fp32.  posk.w = p / rho~^2, vel.w = rho~.
+// which keeps the small excess accurate in fp32.  posk.w = p / rho~^2 (vel.w keeps rho).
 __global__ void __launch_bounds__(256)
-k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, float4 *__restrict__ vel,
+k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const float4 *__restrict__ vel,
             float4 *__restrict__ posk)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -401,7 +403,6 @@ k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, float4 *__restrict__ vel
     float rt = fmaxf(rho, c.rho0);
     float delta = (rt - c.rho0) / c.rho0;
     float pr = c.wc_k * expm1f(c.wc_gamma * log1pf(delta));
-    vel[i].w = rt;
     posk[i] = make_float4(x.x, x.y, x.z, pr / (rt * rt));
 }
 

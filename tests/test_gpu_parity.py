@@ -227,8 +227,14 @@ def test_config2_scaled_rigid_coupling(B, oracle):
 
 def test_config3_scaled_implicit_viscosity(B, oracle):
     """Config 3 at 0.3 scale: matrix-free CG (Eq. 16-19), nu = 10, tol 1e-5."""
+    import torch
     sc = scenes.viscous_column(scale=0.3, steps=8)
     g, o = make_pair(sc, oracle)
+    # the free-falling column has a uniform velocity (A v = 0, CG exits at once): shear it
+    x = g.sph_read_state(B.POS)
+    v0 = torch.zeros_like(x)
+    v0[:, 0] = 2.0 * torch.sin(25.0 * x[:, 2]); v0[:, 1] = 1.5 * torch.cos(30.0 * x[:, 0]); v0[:, 2] = -1.0
+    g.sph_write_state(B.VEL, v0)
     for k in range(6):
         e, st = resync_step(g, o, sc)
         check_errors(e, sc)
