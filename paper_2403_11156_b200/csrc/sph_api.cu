@@ -56,7 +56,8 @@ struct SphSim {
     int *idA = nullptr, *idB = nullptr;
     float *alpha = nullptr;
     GridBufs gf, gb;
-    int *nl_f = nullptr, *nl_b = nullptr, *ncount = nullptr;
+    uint16_t *nl_f = nullptr;       // 16-bit (run, offset) entries, warp-tiled (sph_passes.cuh)
+    int *nl_b = nullptr, *ncount = nullptr;
     float *partial = nullptr, *partial2 = nullptr;
     float4 *cg_r = nullptr, *cg_p = nullptr, *cg_Ap = nullptr;
     // boundary store
@@ -205,7 +206,7 @@ size_t layout(SphSim &s, void *base)
     s.gf.cell_start = w.take<int>(s.cs_len);
     s.gf.ntiles = cdiv((long long)s.cs_len, kScanTile);
     s.gf.tile_sum = w.take<int>((size_t)s.gf.ntiles);
-    s.nl_f = w.take<int>(nwarps * (size_t)s.c.kf * 32);
+    s.nl_f = w.take<uint16_t>(nwarps * (size_t)s.c.kf * 32);
     s.nl_b = w.take<int>(nwarps * (size_t)s.c.kb * 32);
     s.ncount = w.take<int>(nf1);
     s.partial = w.take<float>((size_t)s.nblocks);
@@ -266,16 +267,23 @@ int enqueue_boundary_grid(SphSim *s, cudaStream_t st)
     return enqueue_grid(s, st, s->gb, s->borig_pos, s->borig_vel, nullptr, s->bpos_s, s->bvel_s, s->bid_s, nullptr);
 }
 
-int enqueue_fluid_grid_and_density(SphSim *s, cudaStream_t st)
+// A1-A3 on the fluid, the neighbour lists, then rho and alpha (A4).  divp: also run the P-pass of
+// the first divergence-solve iteration inside the density kernel (DFSPH steps only).
+int enqueue_fluid_grid_and_density(SphSim *s, cudaStream_t st, bool divp)
 {
     int rc = enqueue_grid(s, st, s->gf, s->posA, s->velA, s->idA, s->posB, s->velB, s->idB, &s->stats->oob);
     if (rc) return rc;
     if (s->c.nf > 0) {
         PassCtx p = make_ctx(s);
-        if (s->prm.use_neighbor_list)
-            LAUNCH(s, k_density_alpha<true>, s->nblocks, kBlock, st, p, s->velB, s->alpha, &s->stats->lc);
-        else
-            LAUNCH(s, k_density_alpha<false>, s->nblocks, kBlock, st, p, s->velB, s->alpha, &s->stats->lc);
+        const bool dyn = s->c.has_dynamic != 0;
+        LAUNCH(s, k_build_lists, s->nblocks, kBlock, st, p, &s->stats->lc);
+#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, st, p, s->velB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl)
+        if (s->prm.use_neighbor_list) {
+            if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
+        } else {
+            if (!divp) DENS(false, false, false); else if (dyn) DENS(false, true, true); else DENS(false, true, false);
+        }
+#undef DENS
     }
     return SPH_OK;
 }
@@ -345,8 +353,9 @@ int run_loop(SphSim *s, bool graph_mode, long long *body_counter, Init init, Bod
     return SPH_OK;
 }
 
+// P-pass of one solver iteration
 template <bool LIST>
-int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
 {
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
@@ -357,15 +366,32 @@ int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel
         if (dyn) LAUNCH(s, (k_solver_p<LIST, MODE_DENS, true>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
         else     LAUNCH(s, (k_solver_p<LIST, MODE_DENS, false>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
     }
+    return SPH_OK;
+}
+
+// C-pass, Eq. 14 reactions and the loop predicate of one solver iteration
+template <bool LIST>
+int enqueue_solver_c(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+{
+    PassCtx p = make_ctx(s);
+    const bool dyn = s->c.has_dynamic != 0;
     LAUNCH(s, k_solver_c<LIST>, s->nblocks, kBlock, lc.st, p, s->posk, vel);
     if (dyn && s->ndyn > 0)
         LAUNCH(s, k_boundary_force, cdiv(s->ndyn, kBlock), kBlock, lc.st, s->c, s->dyn_idx, s->ndyn, s->borig_pos,
                s->posk, s->gf.cell_start, s->bforce);
     if (mode == MODE_DIV)
-        LAUNCH(s, k_solver_ctrl<MODE_DIV>, 1, 256, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+        LAUNCH(s, k_solver_ctrl<MODE_DIV>, 1, kCtrlThreads, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
     else
-        LAUNCH(s, k_solver_ctrl<MODE_DENS>, 1, 256, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+        LAUNCH(s, k_solver_ctrl<MODE_DENS>, 1, kCtrlThreads, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
     return SPH_OK;
+}
+
+template <bool LIST>
+int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+{
+    int rc = enqueue_solver_p<LIST>(s, lc, mode, vel);
+    if (rc) return rc;
+    return enqueue_solver_c<LIST>(s, lc, mode, vel);
 }
 
 template <bool LIST>
@@ -381,15 +407,17 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
         if (rc) return rc;
         CUDA_TRY(s, cudaMemsetAsync(s->bforce, 0, sizeof(float4) * (size_t)s->c.nb, st));
     }
-    int rc = enqueue_fluid_grid_and_density(s, st);
+    int rc = enqueue_fluid_grid_and_density(s, st, method == 0);
     if (rc) return rc;
     float4 *vcur = s->velB;
     if (nf > 0) {
         PassCtx p = make_ctx(s);
         if (method == 0) {
-            // divergence-free solve (A5)
+            // divergence-free solve (A5).  The loop is peeled: the P-pass of its first iteration ran
+            // inside k_density_alpha, the first C-pass and predicate follow here, further
+            // iterations (rare under the default tolerance) are the WHILE body.
             rc = run_loop(s, graph_mode, &bc[LOOP_DIV],
-                [&](const LoopCtx &lc) -> int { LAUNCH(s, k_loop_init, 1, 1, lc.st, (int)LOOP_DIV, s->ctl, lc.h, lc.use_handle); return (int)SPH_OK; },
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_c<LIST>(s, lc, MODE_DIV, s->velB); },
                 [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->velB); });
             if (rc) return rc;
             // non-pressure accelerations (A6 / A11)
@@ -402,14 +430,14 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
                     rc = run_loop(s, graph_mode, &bc[LOOP_CG],
                         [&](const LoopCtx &lc) -> int {
                             LAUNCH(s, (k_cg_apply<LIST, true>), s->nblocks, kBlock, lc.st, p, s->velB, s->cg_r, s->cg_p, s->partial, s->partial2);
-                            LAUNCH(s, k_cg_ctrl0, 1, 256, lc.st, s->partial, s->partial2, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+                            LAUNCH(s, k_cg_ctrl0, 1, kCtrlThreads, lc.st, s->partial, s->partial2, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
                             return (int)SPH_OK;
                         },
                         [&](const LoopCtx &lc) -> int {
                             LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, s->cg_p, s->cg_Ap, (float4 *)nullptr, s->partial, (float *)nullptr);
-                            LAUNCH(s, k_cg_ctrl1, 1, 256, lc.st, s->partial, s->nblocks, s->ctl);
+                            LAUNCH(s, k_cg_ctrl1, 1, kCtrlThreads, lc.st, s->partial, s->nblocks, s->ctl);
                             LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->velB, s->cg_r, s->partial2);
-                            LAUNCH(s, k_cg_ctrl2, 1, 256, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);
+                            LAUNCH(s, k_cg_ctrl2, 1, kCtrlThreads, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);
                             LAUNCH(s, k_cg_direction, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_r, s->cg_p);
                             return (int)SPH_OK;
                         });
@@ -543,7 +571,7 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
         CUDA_TRY(s, cudaMemcpyAsync(out, s->idB, bytes, cudaMemcpyDeviceToDevice, st)); break;
     case SPH_FIELD_NEIGHBOR_COUNT: LAUNCH(s, k_export_counts, cdiv(nf, 256), 256, st, s->ncount, s->idB, nf, (int *)out); break;
     case SPH_FIELD_FLUID_NEIGHBORS:
-        LAUNCH(s, k_export_neighbors, cdiv((long long)nf * s->c.kf, 256), 256, st, s->nl_f, s->ncount, 0, s->idB, s->idB, nf, s->c.kf, (int *)out); break;
+        LAUNCH(s, k_export_fluid_neighbors, cdiv((long long)nf * s->c.kf, 256), 256, st, s->nl_f, s->ncount, s->posB, s->c.g, s->gf.cell_start, s->idB, nf, s->c.kf, (int *)out); break;
     case SPH_FIELD_BOUNDARY_NEIGHBORS:
         LAUNCH(s, k_export_neighbors, cdiv((long long)nf * s->c.kb, 256), 256, st, s->nl_b, s->ncount, 16, s->idB, s->bid_s, nf, s->c.kb, (int *)out); break;
     case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->borig_pos, (const int *)nullptr, nb, (float *)out); break;
@@ -708,7 +736,7 @@ int sph_build_grid(SphSim *s)
         int rc = enqueue_boundary_grid(s, st);
         if (rc) return rc;
     }
-    int rc = enqueue_fluid_grid_and_density(s, st);
+    int rc = enqueue_fluid_grid_and_density(s, st, false);
     if (rc) return rc;
     // leave the persistent store sorted as well (the next step's sort is then the identity)
     const size_t nf = (size_t)s->c.nf;

@@ -21,79 +21,155 @@ struct PassCtx {
     const float4 *bpos;
     const int *fcs;     // fluid cell_start [ncells + 1]
     const int *bcs;     // boundary cell_start
-    int *nl_f, *nl_b;   // neighbour lists
+    uint16_t *nl_f;     // fluid neighbour list, 16-bit (x-run, offset) entries (see below)
+    int *nl_b;          // boundary neighbour list, sorted boundary indices
     int *ncount;        // [nf] (#fluid) | (#boundary << 16)
 };
 
 // ---------------------------------------------------------------------------------------------
 // Candidate enumeration: the 27 cells around (cx, cy, cz) as 9 x-runs.  Cells are linearised
 // x-fastest and the store is sorted by cell, so the three x-adjacent cells of one (y, z) row are
-// ONE contiguous index range [cell_start[row + x0], cell_start[row + x1 + 1]).
+// ONE contiguous index range [cell_start[row + x0], cell_start[row + x1 + 1]).  The runs are
+// numbered r = 3 (dz + 1) + (dy + 1); visiting them in this order visits the candidates in
+// ascending sorted index.
+constexpr int kRows = 9;
+constexpr int kOffBits = 12;                 // fluid list entry = (r << 12) | (j - run start)
+constexpr int kOffMask = (1 << kOffBits) - 1;
+
+struct CellOf { int cx, cy, cz, x0, x1; };
+
+__device__ __forceinline__ CellOf cell_of(const Geom &g, float x, float y, float z)
+{
+    CellOf c; bool cl;
+    cell_key(g, x, y, z, cl, c.cx, c.cy, c.cz);
+    c.x0 = max(c.cx - 1, 0); c.x1 = min(c.cx + 1, g.nx - 1);
+    return c;
+}
+
+// first cell of x-run r (index into cell_start), false if the run lies outside the grid
+__device__ __forceinline__ bool run_first_cell(const Geom &g, const CellOf &c, int r, int &first)
+{
+    int z = c.cz + r / 3 - 1, y = c.cy + r % 3 - 1;
+    if ((unsigned)z >= (unsigned)g.nz || (unsigned)y >= (unsigned)g.ny) return false;
+    first = g.nx * (y + g.ny * z) + c.x0;
+    return true;
+}
+
+// f(j, r, s): candidate j of run r whose first index is s
 template <class F>
 __device__ __forceinline__ void for_each_candidate(const Geom &g, const int *__restrict__ cs,
-                                                   int cx, int cy, int cz, F &&f)
+                                                   const CellOf &c, F &&f)
 {
-    int x0 = max(cx - 1, 0), x1 = min(cx + 1, g.nx - 1);
 #pragma unroll 1
-    for (int dz = -1; dz <= 1; ++dz) {
-        int z = cz + dz;
-        if ((unsigned)z >= (unsigned)g.nz) continue;
-#pragma unroll 1
-        for (int dy = -1; dy <= 1; ++dy) {
-            int y = cy + dy;
-            if ((unsigned)y >= (unsigned)g.ny) continue;
-            int row = g.nx * (y + g.ny * z);
-            int s = __ldg(cs + row + x0), e = __ldg(cs + row + x1 + 1);
+    for (int r = 0; r < kRows; ++r) {
+        int first;
+        if (!run_first_cell(g, c, r, first)) continue;
+        int s = __ldg(cs + first), e = __ldg(cs + first + (c.x1 - c.x0) + 1);
 #pragma unroll 4
-            for (int j = s; j < e; ++j) f(j);
-        }
+        for (int j = s; j < e; ++j) f(j, r, s);
     }
 }
 
-// Visit every neighbour of fluid particle i (sorted index), fluid first then boundary:
-//   ff(j, pj, dx, dy, dz, d2) for fluid j != i with d2 < h2,  fb(k, pk, dx, dy, dz, d2) for boundary k;
-//   d = x_i - x_j in fp32, d2 as in reading R10.
-// LIST = true : gather through the per-step list (predicate was evaluated when it was built);
-// LIST = false: walk the cells and evaluate the predicate.
-// `src` is the float4 array whose xyz are the neighbour positions and whose .w the caller wants
-// (pos or posk); WITH_B = false skips the boundary part.
-template <bool LIST, bool WITH_B, class FF, class FB>
+// Fluid neighbour list.  Warp tile w = i / 32 owns kf * 32 16-bit entries; entry k of particle i
+// is at tile + (k >> 1) * 64 + (i & 31) * 2 + (k & 1): a warp reads entries 2p and 2p + 1 of all its
+// lanes with ONE coalesced 128-byte load.  An entry names its neighbour by x-run and offset inside
+// the run, decoded through the particle's table of 9 run starts (tbl, one shared-memory column per
+// thread): j = tbl[r] + off.  Half the bytes of a 32-bit index list: the list is the dominant HBM
+// stream of every solver pass.
+__device__ __forceinline__ size_t list_tile(int i, int cap) { return (size_t)(i >> 5) * (size_t)cap * 32; }
+
+__device__ __forceinline__ void fill_run_table(const Geom &g, const int *__restrict__ cs, const CellOf &c,
+                                               int *tbl /* + threadIdx.x, stride kBlock */)
+{
+#pragma unroll
+    for (int r = 0; r < kRows; ++r) {
+        int first;
+        tbl[r * kBlock] = run_first_cell(g, c, r, first) ? __ldg(cs + first) : 0;
+    }
+}
+
+#ifndef SPH_PAIRS1
+#define SPH_PAIRS1 4      // entry pairs per software-pipeline stage when one array is gathered
+#endif
+#ifndef SPH_PAIRS2
+#define SPH_PAIRS2 2      // ... when two arrays are gathered
+#endif
+
+// Visit every neighbour of fluid particle i (sorted index), fluid first then boundary, both in
+// ascending sorted index:
+//   ff(j, qj, q2j, dx, dy, dz, d2) for fluid j != i with d2 < h2,  fb(k, pk, dx, dy, dz, d2) for boundary k;
+//   d = x_i - x_j in fp32, d2 as in reading R10; qj = src[j], q2j = src2[j] (NSRC == 2, else qj).
+// LIST = true : gather through the per-step list (predicate was evaluated when it was built).  The
+//   list words of the next stage are requested before the gathers of the current one are consumed,
+//   and all gathers of a stage are issued before their arithmetic: the pass is bound by memory
+//   latency otherwise.
+// LIST = false: walk the cells and evaluate the predicate (same visiting order, same arithmetic).
+// `src` is the float4 array whose xyz are the neighbour positions (pos or posk);
+// WITH_B = false skips the boundary part.  tbl: kRows * kBlock ints of shared memory (LIST only).
+template <bool LIST, bool WITH_B, int NSRC, class FF, class FB>
 __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4 *__restrict__ src,
+                                                  const float4 *__restrict__ src2, int *tbl_base,
                                                   int i, float xi, float yi, float zi, FF &&ff, FB &&fb)
 {
+    const CellOf cell = cell_of(p.c.g, xi, yi, zi);
     if (LIST) {
-        int packed = p.ncount[i];
-        int cf = packed & 0xffff, cb = (packed >> 16) & 0xffff;
-        const int *lf = p.nl_f + (size_t)(i >> 5) * p.c.kf * 32 + (i & 31);
-#pragma unroll 4
-        for (int k = 0; k < cf; ++k) {
-            int j = __ldg(lf + k * 32);
-            float4 q = __ldg(src + j);
-            float dx = xi - q.x, dy = yi - q.y, dz = zi - q.z;
-            ff(j, q, dx, dy, dz, dist2_r10(dx, dy, dz));
+        constexpr int PB = NSRC == 2 ? SPH_PAIRS2 : SPH_PAIRS1;
+        const int packed = p.ncount[i];
+        const int cf = packed & 0xffff, cb = (packed >> 16) & 0xffff;
+        int *tbl = tbl_base + threadIdx.x;
+        fill_run_table(p.c.g, p.fcs, cell, tbl);
+        const uint32_t *lp = reinterpret_cast<const uint32_t *>(p.nl_f + list_tile(i, p.c.kf)) + (i & 31);
+        const int npair = (cf + 1) >> 1;
+        uint32_t cur[PB];
+#pragma unroll
+        for (int t = 0; t < PB; ++t) cur[t] = t < npair ? __ldg(lp + t * 32) : 0u;
+#pragma unroll 1
+        for (int pb = 0; pb < npair; pb += PB) {
+            uint32_t nxt[PB];
+#pragma unroll
+            for (int t = 0; t < PB; ++t) nxt[t] = pb + PB + t < npair ? __ldg(lp + (pb + PB + t) * 32) : 0u;
+            int jj[2 * PB];
+            float4 q[2 * PB], q2[NSRC == 2 ? 2 * PB : 1];
+#pragma unroll
+            for (int u = 0; u < 2 * PB; ++u) {
+                const bool valid = 2 * pb + u < cf;
+                uint32_t e = (u & 1) ? (cur[u >> 1] >> 16) : (cur[u >> 1] & 0xffffu);
+                e = valid ? e : 0u;                       // the unwritten half of an odd tail pair is garbage
+                int j = tbl[(e >> kOffBits) * kBlock] + (int)(e & kOffMask);
+                jj[u] = valid ? j : i;
+                q[u] = __ldg(src + jj[u]);
+                if (NSRC == 2) q2[u] = __ldg(src2 + jj[u]);
+            }
+#pragma unroll
+            for (int u = 0; u < 2 * PB; ++u) {
+                if (2 * pb + u < cf) {
+                    float dx = __fsub_rn(xi, q[u].x), dy = __fsub_rn(yi, q[u].y), dz = __fsub_rn(zi, q[u].z);
+                    ff(jj[u], q[u], NSRC == 2 ? q2[u] : q[u], dx, dy, dz, dist2_r10(dx, dy, dz));
+                }
+            }
+#pragma unroll
+            for (int t = 0; t < PB; ++t) cur[t] = nxt[t];
         }
         if (WITH_B && cb > 0) {
-            const int *lb = p.nl_b + (size_t)(i >> 5) * p.c.kb * 32 + (i & 31);
+            const int *lb = p.nl_b + list_tile(i, p.c.kb) + (i & 31);
 #pragma unroll 2
             for (int k = 0; k < cb; ++k) {
                 int j = __ldg(lb + k * 32);
                 float4 q = __ldg(p.bpos + j);
-                float dx = xi - q.x, dy = yi - q.y, dz = zi - q.z;
+                float dx = __fsub_rn(xi, q.x), dy = __fsub_rn(yi, q.y), dz = __fsub_rn(zi, q.z);
                 fb(j, q, dx, dy, dz, dist2_r10(dx, dy, dz));
             }
         }
     } else {
-        bool cl; int cx, cy, cz;
-        cell_key(p.c.g, xi, yi, zi, cl, cx, cy, cz);
         const float h2 = p.c.h2;
-        for_each_candidate(p.c.g, p.fcs, cx, cy, cz, [&](int j) {
+        for_each_candidate(p.c.g, p.fcs, cell, [&](int j, int, int) {
             float4 q = __ldg(src + j);
             float dx = __fsub_rn(xi, q.x), dy = __fsub_rn(yi, q.y), dz = __fsub_rn(zi, q.z);
             float d2 = dist2_r10(dx, dy, dz);
-            if (d2 < h2 && j != i) ff(j, q, dx, dy, dz, d2);
+            if (d2 < h2 && j != i) ff(j, q, NSRC == 2 ? __ldg(src2 + j) : q, dx, dy, dz, d2);
         });
         if (WITH_B && p.c.nb > 0) {
-            for_each_candidate(p.c.g, p.bcs, cx, cy, cz, [&](int j) {
+            for_each_candidate(p.c.g, p.bcs, cell, [&](int j, int, int) {
                 float4 q = __ldg(p.bpos + j);
                 float dx = __fsub_rn(xi, q.x), dy = __fsub_rn(yi, q.y), dz = __fsub_rn(zi, q.z);
                 float d2 = dist2_r10(dx, dy, dz);
@@ -112,57 +188,51 @@ __device__ __forceinline__ float pair_gradf(const SimConst &c, float d2)
 }
 
 // ---------------------------------------------------------------------------------------------
-// A4: density (Eq. 4 + Eq. 12; self term included, R2) and the DFSPH factor
-// alpha_i = rho_i / (|S_i|^2 + T_i), S_i = sum_j m gradW_ij + sum_k Psi_k gradW_ik,
-// T_i = sum_j |m gradW_ij|^2 (R5, R7), in ONE walk of the 27 cells that also writes the
-// neighbour lists every later pass of the step gathers through.
-template <bool WRITE_LIST>
+// A4 first half: ONE walk of the 27 cells per particle per step evaluates the neighbour predicate
+// (R10, bit-exact) and writes the neighbour lists every pass of the step gathers through.  The
+// walk tests ~209 candidates to find ~30 neighbours, so its loop body is kept to the test and a
+// predicated 2-byte store; all arithmetic on neighbours happens in the list passes.
 __global__ void __launch_bounds__(kBlock)
-k_density_alpha(PassCtx p, float4 *__restrict__ vel, float *__restrict__ alpha,
-                ListCounters *__restrict__ lc)
+k_build_lists(PassCtx p, ListCounters *__restrict__ lc)
 {
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     int cf = 0, cb = 0;
+    bool ovf = false;
     if (i < c.nf) {
         float4 xi = p.pos[i];
-        float sw = 0.f, sx = 0.f, sy = 0.f, sz = 0.f, t2 = 0.f;    // fluid: sum w, sum gf d, sum gf^2 d2
-        float bw = 0.f, bx = 0.f, by = 0.f, bz = 0.f;              // boundary, Psi-weighted
-        int *lf = p.nl_f + (size_t)(i >> 5) * c.kf * 32 + (i & 31);
-        int *lb = p.nl_b + (size_t)(i >> 5) * c.kb * 32 + (i & 31);
-        for_each_neighbor<false, true>(p, p.pos, i, xi.x, xi.y, xi.z,
-            [&](int j, float4, float dx, float dy, float dz, float d2) {
-                float r, rinv;
-                r_and_rinv(d2, r, rinv);
-                float q = r * c.inv_h;
-                sw += spline_w(q);
-                float gf = spline_gradf(q, rinv, c.inv_h);
-                sx = fmaf(gf, dx, sx); sy = fmaf(gf, dy, sy); sz = fmaf(gf, dz, sz);
-                t2 = fmaf(gf * gf, d2, t2);
-                if (WRITE_LIST && cf < c.kf) lf[cf * 32] = j;
-                ++cf;
-            },
-            [&](int k, float4 pk, float dx, float dy, float dz, float d2) {
-                float r, rinv;
-                r_and_rinv(d2, r, rinv);
-                float q = r * c.inv_h;
-                bw = fmaf(pk.w, spline_w(q), bw);
-                float gf = pk.w * spline_gradf(q, rinv, c.inv_h);
-                bx = fmaf(gf, dx, bx); by = fmaf(gf, dy, by); bz = fmaf(gf, dz, bz);
-                if (WRITE_LIST && cb < c.kb) lb[cb * 32] = k;
-                ++cb;
+        const CellOf cell = cell_of(c.g, xi.x, xi.y, xi.z);
+        const float h2 = c.h2;
+        uint16_t *lf = p.nl_f + list_tile(i, c.kf) + (i & 31) * 2;
+        for_each_candidate(c.g, p.fcs, cell, [&](int j, int r, int s) {
+            float4 q = __ldg(p.pos + j);
+            float dx = __fsub_rn(xi.x, q.x), dy = __fsub_rn(xi.y, q.y), dz = __fsub_rn(xi.z, q.z);
+            float d2 = dist2_r10(dx, dy, dz);
+            if (d2 < h2 && j != i) {
+                int off = j - s;
+                if (off > kOffMask) ovf = true;
+                else {
+                    if (cf < c.kf) lf[(cf >> 1) * 64 + (cf & 1)] = (uint16_t)((r << kOffBits) | off);
+                    ++cf;
+                }
+            }
+        });
+        if (c.nb > 0) {
+            int *lb = p.nl_b + list_tile(i, c.kb) + (i & 31);
+            for_each_candidate(c.g, p.bcs, cell, [&](int k, int, int) {
+                float4 q = __ldg(p.bpos + k);
+                float dx = __fsub_rn(xi.x, q.x), dy = __fsub_rn(xi.y, q.y), dz = __fsub_rn(xi.z, q.z);
+                float d2 = dist2_r10(dx, dy, dz);
+                if (d2 < h2) {
+                    if (cb < c.kb) lb[cb * 32] = k;
+                    ++cb;
+                }
             });
-        float rho = c.sigma * fmaf(c.m, 1.0f + sw, bw);            // W(0) = sigma
-        float Sx = c.grad_c * fmaf(c.m, sx, bx), Sy = c.grad_c * fmaf(c.m, sy, by),
-              Sz = c.grad_c * fmaf(c.m, sz, bz);
-        float T = (c.grad_c * c.m) * (c.grad_c * c.m) * t2;
-        float den = fmaf(Sx, Sx, fmaf(Sy, Sy, fmaf(Sz, Sz, T)));
-        alpha[i] = den > 1e-6f ? rho / den : 0.0f;
-        vel[i].w = rho;
+        }
         p.ncount[i] = min(cf, c.kf) | (min(cb, c.kb) << 16);
+        ovf = ovf || cf > c.kf || cb > c.kb;
     }
     // statistics: overflow count, maxima, mean neighbour count (warp-aggregated atomics)
-    bool ovf = (i < c.nf) && (cf > c.kf || cb > c.kb);
     unsigned bo = __ballot_sync(0xffffffffu, ovf);
     int mf = cf, mb = cb, sf = cf;
 #pragma unroll
@@ -180,13 +250,93 @@ k_density_alpha(PassCtx p, float4 *__restrict__ vel, float *__restrict__ alpha,
 }
 
 // ---------------------------------------------------------------------------------------------
+// A4 second half: density (Eq. 4 + Eq. 12; self term included, R2) and the
+// DFSPH factor alpha_i = rho_i / (|S_i|^2 + T_i), S_i = sum_j m gradW_ij + sum_k Psi_k gradW_ik,
+// T_i = sum_j |m gradW_ij|^2 (R5, R7).
+// DIVP = true additionally runs the P-pass of the FIRST divergence-solve iteration in the same
+// neighbour loop (A5): D_i needs only the velocities of the step's start, and kappa^v_i the
+// alpha_i that this very loop produces -- one full neighbour pass less per step.  It writes
+// posk[i] = (x_i, kappa^v_i / rho_i) (0 when the divergence solve is switched off) and the CTA
+// partial of R_i = max(D_i, 0).
+enum { MODE_DIV = 0, MODE_DENS = 1 };
+
+template <bool LIST, bool DIVP, bool DYN>
+__global__ void __launch_bounds__(kBlock)
+k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ bvel,
+                float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
+                const DevControl *__restrict__ ctl)
+{
+    __shared__ float red[kBlock / 32];
+    __shared__ int tbl[LIST ? kRows * kBlock : 1];
+    const SimConst &c = p.c;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float term = 0.f;
+    if (i < c.nf) {
+        float4 xi = p.pos[i];
+        float4 vi = vel[i];
+        float sw = 0.f, sx = 0.f, sy = 0.f, sz = 0.f, t2 = 0.f;    // fluid: sum w, sum gf d, sum gf^2 d2
+        float bw = 0.f, bx = 0.f, by = 0.f, bz = 0.f;              // boundary, Psi-weighted
+        float df = 0.f, db = 0.f;                                  // density rate (DIVP)
+        for_each_neighbor<LIST, true, DIVP ? 2 : 1>(p, p.pos, vel, tbl, i, xi.x, xi.y, xi.z,
+            [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
+                float r, rinv;
+                r_and_rinv(d2, r, rinv);
+                float q = r * c.inv_h;
+                sw += spline_w(q);
+                float gf = spline_gradf(q, rinv, c.inv_h);
+                sx = fmaf(gf, dx, sx); sy = fmaf(gf, dy, sy); sz = fmaf(gf, dz, sz);
+                t2 = fmaf(gf * gf, d2, t2);
+                if (DIVP) {
+                    float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
+                    df = fmaf(gf, dv, df);
+                }
+            },
+            [&](int k, float4 pk, float dx, float dy, float dz, float d2) {
+                float r, rinv;
+                r_and_rinv(d2, r, rinv);
+                float q = r * c.inv_h;
+                bw = fmaf(pk.w, spline_w(q), bw);
+                float gf = pk.w * spline_gradf(q, rinv, c.inv_h);
+                bx = fmaf(gf, dx, bx); by = fmaf(gf, dy, by); bz = fmaf(gf, dz, bz);
+                if (DIVP) {
+                    float dv;
+                    if (DYN) {
+                        float4 vk = __ldg(bvel + k);
+                        dv = fmaf(vi.x - vk.x, dx, fmaf(vi.y - vk.y, dy, (vi.z - vk.z) * dz));
+                    } else dv = fmaf(vi.x, dx, fmaf(vi.y, dy, vi.z * dz));
+                    db = fmaf(gf, dv, db);
+                }
+            });
+        float rho = c.sigma * fmaf(c.m, 1.0f + sw, bw);            // W(0) = sigma
+        float Sx = c.grad_c * fmaf(c.m, sx, bx), Sy = c.grad_c * fmaf(c.m, sy, by),
+              Sz = c.grad_c * fmaf(c.m, sz, bz);
+        float T = (c.grad_c * c.m) * (c.grad_c * c.m) * t2;
+        float den = fmaf(Sx, Sx, fmaf(Sy, Sy, fmaf(Sz, Sz, T)));
+        float a = den > 1e-6f ? rho / den : 0.0f;
+        alpha[i] = a;
+        vel[i].w = rho;   // 4-byte store: concurrent gathers of vel[i] by other threads use xyz only
+        if (DIVP) {
+            // Eq. 10 source (R15): R_i = max(D_i, 0), kappa^v_i = alpha_i R_i / dt
+            bool on = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;
+            float D = c.grad_c * fmaf(c.m, df, db);
+            term = fmaxf(D, 0.f);
+            float kappa = a * term / c.dt;
+            posk[i] = make_float4(xi.x, xi.y, xi.z, on ? kappa / rho : 0.f);
+        }
+    }
+    if (DIVP) {
+        float s = block_sum(term, red);
+        if (threadIdx.x == 0) partial[blockIdx.x] = s;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // P-pass of both solvers (A5 / A7).  Density rate (Eq. 6 times rho):
 //   D_i = sum_j m (v_i - v_j).gradW_ij + sum_k Psi_k (v_i - v_k).gradW_ik
 // DIV  (Eq. 10 source; R15): R_i = max(D_i, 0), kappa^v_i = alpha_i R_i / dt, term = R_i
 // DENS (Eq. 8-9; R15) : E_i = max(rho_i + dt D_i, rho0) - rho0,
 //                                          kappa_i = alpha_i E_i / dt^2, term = E_i
 // Writes posk[i] = (x_i, kappa_i / rho_i) and one partial sum of `term` per CTA.
-enum { MODE_DIV = 0, MODE_DENS = 1 };
 
 template <bool LIST, int MODE, bool DYN>
 __global__ void __launch_bounds__(kBlock)
@@ -194,6 +344,7 @@ k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__
            const float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial)
 {
     __shared__ float red[kBlock / 32];
+    __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     float term = 0.f;
@@ -201,9 +352,8 @@ k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__
         float4 xi = p.pos[i];
         float4 vi = vel[i];
         float df = 0.f, db = 0.f;
-        for_each_neighbor<LIST, true>(p, p.pos, i, xi.x, xi.y, xi.z,
-            [&](int j, float4, float dx, float dy, float dz, float d2) {
-                float4 vj = __ldg(vel + j);
+        for_each_neighbor<LIST, true, 2>(p, p.pos, vel, tbl, i, xi.x, xi.y, xi.z,
+            [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
                 float gf = pair_gradf(c, d2);
                 float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
                 df = fmaf(gf, dv, df);
@@ -238,14 +388,15 @@ template <bool LIST>
 __global__ void __launch_bounds__(kBlock)
 k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel)
 {
+    __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.nf) return;
     float4 xi = posk[i];
     float kri = xi.w;
     float fx = 0.f, fy = 0.f, fz = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-    for_each_neighbor<LIST, true>(p, posk, i, xi.x, xi.y, xi.z,
-        [&](int, float4 pj, float dx, float dy, float dz, float d2) {
+    for_each_neighbor<LIST, true, 1>(p, posk, posk, tbl, i, xi.x, xi.y, xi.z,
+        [&](int, float4 pj, float4, float dx, float dy, float dz, float d2) {
             float s = (kri + pj.w) * pair_gradf(c, d2);
             fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz);
         },
@@ -282,15 +433,15 @@ template <bool LIST, bool CLAMP>
 __global__ void __launch_bounds__(kBlock)
 k_explicit_viscosity(PassCtx p, const float4 *__restrict__ vin, float4 *__restrict__ vout)
 {
+    __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.nf) return;
     float4 xi = p.pos[i];
     float4 vi = vin[i];
     float ax = 0.f, ay = 0.f, az = 0.f;
-    for_each_neighbor<LIST, false>(p, p.pos, i, xi.x, xi.y, xi.z,
-        [&](int j, float4, float dx, float dy, float dz, float d2) {
-            float4 vj = __ldg(vin + j);
+    for_each_neighbor<LIST, false, 2>(p, p.pos, vin, tbl, i, xi.x, xi.y, xi.z,
+        [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
             float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
             float rj = CLAMP ? fmaxf(vj.w, c.rho0) : vj.w;
             float s = pair_gradf(c, d2) * dv / ((d2 + c.visc_eps) * rj);
@@ -317,6 +468,7 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u, float4 *__restrict__ out,
            float4 *__restrict__ out2, float *__restrict__ partial, float *__restrict__ partial2)
 {
     __shared__ float red[kBlock / 32];
+    __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     float t1 = 0.f, t2 = 0.f;
@@ -324,9 +476,8 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u, float4 *__restrict__ out,
         float4 xi = p.pos[i];
         float4 ui = u[i];
         float ax = 0.f, ay = 0.f, az = 0.f;
-        for_each_neighbor<LIST, false>(p, p.pos, i, xi.x, xi.y, xi.z,
-            [&](int j, float4, float dx, float dy, float dz, float d2) {
-                float4 uj = __ldg(u + j);
+        for_each_neighbor<LIST, false, 2>(p, p.pos, u, tbl, i, xi.x, xi.y, xi.z,
+            [&](int, float4, float4 uj, float dx, float dy, float dz, float d2) {
                 float du = fmaf(ui.x - uj.x, dx, fmaf(ui.y - uj.y, dy, (ui.z - uj.z) * dz));
                 float s = pair_gradf(c, d2) * du / ((d2 + c.visc_eps) * uj.w);
                 ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay); az = fmaf(s, dz, az);
@@ -443,9 +594,16 @@ k_integrate(SimConst c, const float4 *__restrict__ pos, const float4 *__restrict
 // is tested after its C-pass) and sets the CUDA-graph WHILE condition -- no host round trip.
 __device__ __forceinline__ double reduce_partials(const float *__restrict__ partial, int n, double *sm)
 {
-    double s = 0.0;
-    for (int k = threadIdx.x; k < n; k += blockDim.x) s += (double)partial[k];
-    return block_sum(s, sm);
+    // fixed summation order (deterministic): four independent strided chains per thread
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    const int st = blockDim.x;
+    int k = threadIdx.x;
+    for (; k + 3 * st < n; k += 4 * st) {
+        float a = partial[k], b = partial[k + st], c = partial[k + 2 * st], d = partial[k + 3 * st];
+        s0 += (double)a; s1 += (double)b; s2 += (double)c; s3 += (double)d;
+    }
+    for (; k < n; k += st) s0 += (double)partial[k];
+    return block_sum((s0 + s1) + (s2 + s3), sm);
 }
 
 __device__ __forceinline__ void set_loop_condition(cudaGraphConditionalHandle h, int use_handle,

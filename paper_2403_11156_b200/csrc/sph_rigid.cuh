@@ -64,7 +64,29 @@ k_export_counts(const int *__restrict__ ncount, const int *__restrict__ id, int 
     out[2 * id[s]] = p & 0xffff;
     out[2 * id[s] + 1] = (p >> 16) & 0xffff;
 }
-// neighbour rows in caller ids, -1 padded: out[id[s]*K + k] = nid[list entry k of s]
+// fluid neighbour rows in caller ids, -1 padded: 16-bit (run, offset) entries decoded through the
+// particle's run starts (sph_passes.cuh)
+__global__ void __launch_bounds__(256)
+k_export_fluid_neighbors(const uint16_t *__restrict__ nl, const int *__restrict__ ncount,
+                         const float4 *__restrict__ pos, Geom g, const int *__restrict__ fcs,
+                         const int *__restrict__ id, int n, int K, int *__restrict__ out)
+{
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n * K) return;
+    int s = (int)(t / K), k = (int)(t % K);
+    int cnt = ncount[s] & 0xffff;
+    int v = -1;
+    if (k < cnt) {
+        unsigned e = nl[list_tile(s, K) + (size_t)(k >> 1) * 64 + (s & 31) * 2 + (k & 1)];
+        float4 x = pos[s];
+        CellOf c = cell_of(g, x.x, x.y, x.z);
+        int first;
+        if (run_first_cell(g, c, (int)(e >> kOffBits), first)) v = id[fcs[first] + (int)(e & kOffMask)];
+    }
+    out[(size_t)id[s] * K + k] = v;
+}
+
+// boundary neighbour rows in caller ids, -1 padded: out[id[s]*K + k] = nid[list entry k of s]
 __global__ void __launch_bounds__(256)
 k_export_neighbors(const int *__restrict__ nl, const int *__restrict__ ncount, int shift,
                    const int *__restrict__ id, const int *__restrict__ nid, int n, int K,
@@ -125,10 +147,9 @@ k_boundary_psi(SimConst c, float4 *__restrict__ bpos_s, const int *__restrict__ 
     if (s >= c.nb) return;
     float4 x = bpos_s[s];
     int me = bid_s[s], body = bbody[me];
-    bool cl; int cx, cy, cz;
-    cell_key(c.g, x.x, x.y, x.z, cl, cx, cy, cz);
+    const CellOf cell = cell_of(c.g, x.x, x.y, x.z);
     float sw = 0.f;
-    for_each_candidate(c.g, bcs, cx, cy, cz, [&](int j) {
+    for_each_candidate(c.g, bcs, cell, [&](int j, int, int) {
         if (j == s) return;
         float4 q = bpos_s[j];
         float dx = __fsub_rn(x.x, q.x), dy = __fsub_rn(x.y, q.y), dz = __fsub_rn(x.z, q.z);
@@ -157,10 +178,9 @@ k_boundary_force(SimConst c, const int *__restrict__ dyn_idx, int ndyn,
     if (t >= ndyn) return;
     int k = dyn_idx[t];
     float4 xk = bpos_orig[k];
-    bool cl; int cx, cy, cz;
-    cell_key(c.g, xk.x, xk.y, xk.z, cl, cx, cy, cz);
+    const CellOf cell = cell_of(c.g, xk.x, xk.y, xk.z);
     float fx = 0.f, fy = 0.f, fz = 0.f;
-    for_each_candidate(c.g, fcs, cx, cy, cz, [&](int i) {
+    for_each_candidate(c.g, fcs, cell, [&](int i, int, int) {
         float4 q = __ldg(posk + i);
         float dx = __fsub_rn(q.x, xk.x), dy = __fsub_rn(q.y, xk.y), dz = __fsub_rn(q.z, xk.z);  // x_i - x_k
         float d2 = dist2_r10(dx, dy, dz);
@@ -256,6 +276,7 @@ k_rigid_step(SimConst c, SphRigidBody *__restrict__ bodies, float tminx, float t
 // ---------------------------------------------------------------------------------------------
 // A12 loop control kernels (single CTA each).
 enum { LOOP_DIV = 0, LOOP_DENS = 1, LOOP_CG = 2 };
+constexpr int kCtrlThreads = 1024;   // one CTA sums the per-CTA partials: wide, so that the loads overlap
 
 __global__ void k_step_begin(DevStats *st, DevControl *ctl)
 {
@@ -281,22 +302,28 @@ __global__ void k_loop_init(int kind, DevControl *ctl, cudaGraphConditionalHandl
 {
     ctl->it = 0;
     int cont;
-    if (kind == LOOP_DIV) cont = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;
+    if (kind == LOOP_DIV) cont = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;   // (unused: the divergence loop is peeled)
     else cont = ctl->forced_d != 0 && ctl->max_d > 0;
     set_loop_condition(h, use_handle, ctl, cont);
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kCtrlThreads)
 k_solver_ctrl(SimConst c, const float *__restrict__ partial, int nparts, DevControl *ctl,
               DevStats *st, cudaGraphConditionalHandle h, int use_handle)
 {
-    __shared__ double sm[8];
+    __shared__ double sm[kCtrlThreads / 32];
     double sum = reduce_partials(partial, nparts, sm);
     if (threadIdx.x != 0) return;
     double mean = c.nf > 0 ? sum / (double)c.nf : 0.0;
-    int l = ++ctl->it;
     int cont;
+    if (MODE == MODE_DIV && !(ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0)) {
+        // divergence solve switched off: the peeled first iteration ran with kappa^v = 0 (a no-op)
+        st->it_v = 0; st->err_v = 0.f;
+        set_loop_condition(h, use_handle, ctl, 0);
+        return;
+    }
+    int l = ++ctl->it;
     if (MODE == MODE_DIV) {
         double err = (double)c.dt / (double)c.rho0 * mean;     // R6: density change per step
         int f = ctl->forced_v;
@@ -314,11 +341,11 @@ k_solver_ctrl(SimConst c, const float *__restrict__ partial, int nparts, DevCont
 }
 
 // CG start: |b|^2, |r0|^2, first predicate (R23: stop when |r| <= tol |b| or max iterations)
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kCtrlThreads)
 k_cg_ctrl0(const float *__restrict__ pbb, const float *__restrict__ prr, int nparts, DevControl *ctl,
            DevStats *st, cudaGraphConditionalHandle h, int use_handle)
 {
-    __shared__ double sm[8];
+    __shared__ double sm[kCtrlThreads / 32];
     double bb = reduce_partials(pbb, nparts, sm);
     double rr = reduce_partials(prr, nparts, sm);
     if (threadIdx.x != 0) return;
@@ -331,21 +358,21 @@ k_cg_ctrl0(const float *__restrict__ pbb, const float *__restrict__ prr, int npa
     set_loop_condition(h, use_handle, ctl, cont);
 }
 // alpha = rr / pAp
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kCtrlThreads)
 k_cg_ctrl1(const float *__restrict__ ppap, int nparts, DevControl *ctl)
 {
-    __shared__ double sm[8];
+    __shared__ double sm[kCtrlThreads / 32];
     double pAp = reduce_partials(ppap, nparts, sm);
     if (threadIdx.x != 0) return;
     if (!(pAp > 0.0)) { ctl->cg_alpha = 0.0; ctl->cg_break = 1; }
     else ctl->cg_alpha = ctl->cg_rr / pAp;
 }
 // beta = rr_new / rr, iteration count, predicate
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kCtrlThreads)
 k_cg_ctrl2(const float *__restrict__ prr, int nparts, DevControl *ctl, DevStats *st,
            cudaGraphConditionalHandle h, int use_handle)
 {
-    __shared__ double sm[8];
+    __shared__ double sm[kCtrlThreads / 32];
     double rr_new = reduce_partials(prr, nparts, sm);
     if (threadIdx.x != 0) return;
     int cont = 0;
