@@ -73,7 +73,8 @@ typedef struct SphParams {
     float wcsph_stiffness;     /* k */
     float wcsph_exponent;      /* gamma */
     int   max_fluid_neighbors;    /* capacity of the per-particle fluid neighbour list, 0 => 64;
-                                     rounded up to a multiple of 4.  Overflow is counted in
+                                     rounded up to a multiple of 4, at most 768 (the list builder
+                                     stages a warp's lists in shared memory).  Overflow is counted in
                                      SphStats.overflow_count and the step's results are invalid */
     int   max_boundary_neighbors; /* same for boundary neighbours, 0 => 64 */
     int   use_cuda_graph;      /* 1: one CUDA graph per step with device-side WHILE loops (default

@@ -154,7 +154,7 @@ bool make_geom(const SphParams &p, Geom &g, std::string &why)
     return true;
 }
 
-int list_cap(int v) { if (v <= 0) v = 64; v = (v + 3) & ~3; if (v > 65532) v = 65532; return v; }
+int list_cap(int v, int vmax) { if (v <= 0) v = 64; v = (v + 3) & ~3; if (v > vmax) v = vmax; return v; }
 
 bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &why)
 {
@@ -164,8 +164,8 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     }
     if (!make_geom(p, c.g, why)) return false;
     c.nf = nf; c.nb = nb;
-    c.kf = list_cap(p.max_fluid_neighbors);
-    c.kb = list_cap(p.max_boundary_neighbors);
+    c.kf = list_cap(p.max_fluid_neighbors, kMaxListCap);
+    c.kb = list_cap(p.max_boundary_neighbors, 65532);
     c.h = p.support_radius;
     c.h2 = c.h * c.h;                                   // fp32 product (R10)
     c.inv_h = 1.0f / c.h;
@@ -197,7 +197,7 @@ size_t layout(SphSim &s, void *base)
     s.ctl = w.take<DevControl>(1);
     s.stats = w.take<DevStats>(1);
     s.posA = w.take<float4>(nf1); s.velA = w.take<float4>(nf1); s.idA = w.take<int>(nf1);
-    s.posB = w.take<float4>(nf1); s.velB = w.take<float4>(nf1); s.idB = w.take<int>(nf1);
+    s.posB = w.take<float4>(nf1 + kPosPad); s.velB = w.take<float4>(nf1); s.idB = w.take<int>(nf1);
     s.velC = s.prm.viscosity_mode == 1 ? w.take<float4>(nf1) : nullptr;
     s.posk = w.take<float4>(nf1);
     s.alpha = w.take<float>(nf1);
@@ -276,7 +276,17 @@ int enqueue_fluid_grid_and_density(SphSim *s, cudaStream_t st, bool divp)
     if (s->c.nf > 0) {
         PassCtx p = make_ctx(s);
         const bool dyn = s->c.has_dynamic != 0;
-        LAUNCH(s, k_build_lists, s->nblocks, kBlock, st, p, &s->stats->lc);
+        {
+            // staging rows of the list builder: kf + kStageExtra rows of 32 16-bit entries per warp
+            const int rows = s->c.kf + kStageExtra;
+            const size_t smem = (size_t)rows * 64 * (kBlock / 32);
+            cudaEvent_t ea_ = nullptr, eb_ = nullptr;
+            if (s->timing) { ea_ = take_event(s); eb_ = take_event(s); cudaEventRecord(ea_, st); }
+            k_build_lists<<<s->nblocks, kBlock, smem, st>>>(p, &s->stats->lc, rows);
+            if (s->timing) { cudaEventRecord(eb_, st); s->timed.push_back({ "k_build_lists", ea_, eb_ }); }
+            ++*s->cur_counter;
+            CUDA_TRY(s, cudaGetLastError());
+        }
 #define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, st, p, s->velB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl)
         if (s->prm.use_neighbor_list) {
             if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
@@ -625,7 +635,7 @@ int sph_grid_dims(const SphParams *params, int dims[4], int caps[2])
     std::string why;
     if (!make_geom(*params, g, why)) return SPH_EDOMAIN;
     if (dims) { dims[0] = g.nx; dims[1] = g.ny; dims[2] = g.nz; dims[3] = g.ncells; }
-    if (caps) { caps[0] = list_cap(params->max_fluid_neighbors); caps[1] = list_cap(params->max_boundary_neighbors); }
+    if (caps) { caps[0] = list_cap(params->max_fluid_neighbors, kMaxListCap); caps[1] = list_cap(params->max_boundary_neighbors, 65532); }
     return SPH_OK;
 }
 
@@ -670,6 +680,8 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
         cudaStream_t st = s->stream;
         CUDA_TRY(s, cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
         CUDA_TRY(s, cudaMallocHost(&s->pinned, 4096));
+        CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (kMaxListCap + kStageExtra) * 64 * (kBlock / 32)));
         const int nf = s->c.nf, nb = s->c.nb;
         // control + statistics blocks
         DevControl hc;
