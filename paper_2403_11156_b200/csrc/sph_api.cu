@@ -267,38 +267,6 @@ int enqueue_boundary_grid(SphSim *s, cudaStream_t st)
     return enqueue_grid(s, st, s->gb, s->borig_pos, s->borig_vel, nullptr, s->bpos_s, s->bvel_s, s->bid_s, nullptr);
 }
 
-// A1-A3 on the fluid, the neighbour lists, then rho and alpha (A4).  divp: also run the P-pass of
-// the first divergence-solve iteration inside the density kernel (DFSPH steps only).
-int enqueue_fluid_grid_and_density(SphSim *s, cudaStream_t st, bool divp)
-{
-    int rc = enqueue_grid(s, st, s->gf, s->posA, s->velA, s->idA, s->posB, s->velB, s->idB, &s->stats->oob);
-    if (rc) return rc;
-    if (s->c.nf > 0) {
-        PassCtx p = make_ctx(s);
-        const bool dyn = s->c.has_dynamic != 0;
-        {
-            // staging rows of the list builder: kf + kStageExtra rows of 32 16-bit entries per warp
-            const int rows = s->c.kf + kStageExtra;
-            const size_t smem = (size_t)rows * 64 * (kBlock / 32);
-            cudaEvent_t ea_ = nullptr, eb_ = nullptr;
-            if (s->timing) { ea_ = take_event(s); eb_ = take_event(s); cudaEventRecord(ea_, st); }
-            k_build_lists<<<s->nblocks, kBlock, smem, st>>>(p, &s->stats->lc, rows);
-            if (s->timing) { cudaEventRecord(eb_, st); s->timed.push_back({ "k_build_lists", ea_, eb_ }); }
-            ++*s->cur_counter;
-            CUDA_TRY(s, cudaGetLastError());
-        }
-#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, st, p, s->velB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl)
-        if (s->prm.use_neighbor_list) {
-            if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
-        } else {
-            if (!divp) DENS(false, false, false); else if (dyn) DENS(false, true, true); else DENS(false, true, false);
-        }
-#undef DENS
-    }
-    return SPH_OK;
-}
-
-// ------------------------------------------------------------------------------------------
 // Solver loops.  graph mode: a conditional WHILE node whose body is captured on the helper
 // stream; host mode: the host reads the predicate after every iteration.
 struct LoopCtx {
@@ -306,6 +274,46 @@ struct LoopCtx {
     cudaGraphConditionalHandle h;
     int use_handle;
 };
+
+// A1-A3 on the fluid, then the neighbour lists (A4 first half).
+int enqueue_fluid_grid_and_lists(SphSim *s, cudaStream_t st)
+{
+    int rc = enqueue_grid(s, st, s->gf, s->posA, s->velA, s->idA, s->posB, s->velB, s->idB, &s->stats->oob);
+    if (rc) return rc;
+    if (s->c.nf > 0) {
+        PassCtx p = make_ctx(s);
+        // staging rows of the list builder: kf + kStageExtra rows of 32 16-bit entries per warp
+        const int rows = s->c.kf + kStageExtra;
+        const size_t smem = (size_t)rows * 64 * (kBlock / 32);
+        cudaEvent_t ea_ = nullptr, eb_ = nullptr;
+        if (s->timing) { ea_ = take_event(s); eb_ = take_event(s); cudaEventRecord(ea_, st); }
+        k_build_lists<<<s->nblocks, kBlock, smem, st>>>(p, &s->stats->lc, rows);
+        if (s->timing) { cudaEventRecord(eb_, st); s->timed.push_back({ "k_build_lists", ea_, eb_ }); }
+        ++*s->cur_counter;
+        CUDA_TRY(s, cudaGetLastError());
+    }
+    return SPH_OK;
+}
+
+// rho and alpha (A4 second half).  divp: also the P-pass of the first divergence-solve iteration
+// and, in its last CTA, the loop predicate (DFSPH steps only).
+int enqueue_density(SphSim *s, const LoopCtx &lc, bool divp)
+{
+    if (s->c.nf <= 0) return SPH_OK;
+    PassCtx p = make_ctx(s);
+    const bool dyn = s->c.has_dynamic != 0;
+    LoopHandle lh{ lc.h, lc.use_handle };
+#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->velB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl, s->stats, lh)
+    if (s->prm.use_neighbor_list) {
+        if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
+    } else {
+        if (!divp) DENS(false, false, false); else if (dyn) DENS(false, true, true); else DENS(false, true, false);
+    }
+#undef DENS
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------
 
 int read_cont(SphSim *s, int *cont)
 {
@@ -363,45 +371,46 @@ int run_loop(SphSim *s, bool graph_mode, long long *body_counter, Init init, Bod
     return SPH_OK;
 }
 
-// P-pass of one solver iteration
+// P-pass of one solver iteration (its last CTA evaluates the loop predicate, A12)
 template <bool LIST>
-int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, float4 *vel, int first)
 {
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
-    if (mode == MODE_DIV) {
-        if (dyn) LAUNCH(s, (k_solver_p<LIST, MODE_DIV, true>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
-        else     LAUNCH(s, (k_solver_p<LIST, MODE_DIV, false>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
-    } else {
-        if (dyn) LAUNCH(s, (k_solver_p<LIST, MODE_DENS, true>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
-        else     LAUNCH(s, (k_solver_p<LIST, MODE_DENS, false>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial);
-    }
+    LoopHandle lh{ lc.h, lc.use_handle };
+#define SOLP(MODE, DYN) LAUNCH(s, (k_solver_p<LIST, MODE, DYN>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl, s->stats, lh, first)
+    if (mode == MODE_DIV) { if (dyn) SOLP(MODE_DIV, true); else SOLP(MODE_DIV, false); }
+    else                  { if (dyn) SOLP(MODE_DENS, true); else SOLP(MODE_DENS, false); }
+#undef SOLP
     return SPH_OK;
 }
 
-// C-pass, Eq. 14 reactions and the loop predicate of one solver iteration
+// C-pass (with the tail work of the loop's last iteration) and the Eq. 14 reactions
 template <bool LIST>
-int enqueue_solver_c(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, float4 *vel)
 {
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
-    LAUNCH(s, k_solver_c<LIST>, s->nblocks, kBlock, lc.st, p, s->posk, vel);
+    CTail t;
+    t.ctl = s->ctl;
+    t.add_gravity = s->prm.viscosity_mode != 1;
+    t.id = s->idB; t.pos_out = s->posA; t.vel_out = s->velA; t.id_out = s->idA;
+    t.vmax_bits = &s->stats->vmax_bits; t.nan_count = &s->stats->nan_count;
+    if (tail == TAIL_DIV)       LAUNCH(s, (k_solver_c<LIST, TAIL_DIV>), s->nblocks, kBlock, st, p, s->posk, vel, t);
+    else if (tail == TAIL_DENS) LAUNCH(s, (k_solver_c<LIST, TAIL_DENS>), s->nblocks, kBlock, st, p, s->posk, vel, t);
+    else                        LAUNCH(s, (k_solver_c<LIST, TAIL_WCSPH>), s->nblocks, kBlock, st, p, s->posk, vel, t);
     if (dyn && s->ndyn > 0)
-        LAUNCH(s, k_boundary_force, cdiv(s->ndyn, kBlock), kBlock, lc.st, s->c, s->dyn_idx, s->ndyn, s->borig_pos,
+        LAUNCH(s, k_boundary_force, cdiv(s->ndyn, kBlock), kBlock, st, s->c, s->dyn_idx, s->ndyn, s->borig_pos,
                s->posk, s->gf.cell_start, s->bforce);
-    if (mode == MODE_DIV)
-        LAUNCH(s, k_solver_ctrl<MODE_DIV>, 1, kCtrlThreads, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
-    else
-        LAUNCH(s, k_solver_ctrl<MODE_DENS>, 1, kCtrlThreads, lc.st, s->c, s->partial, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
     return SPH_OK;
 }
 
 template <bool LIST>
-int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel)
+int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel, int first)
 {
-    int rc = enqueue_solver_p<LIST>(s, lc, mode, vel);
+    int rc = enqueue_solver_p<LIST>(s, lc, mode, vel, first);
     if (rc) return rc;
-    return enqueue_solver_c<LIST>(s, lc, mode, vel);
+    return enqueue_solver_c<LIST>(s, lc.st, mode == MODE_DIV ? TAIL_DIV : TAIL_DENS, vel);
 }
 
 template <bool LIST>
@@ -417,64 +426,63 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
         if (rc) return rc;
         CUDA_TRY(s, cudaMemsetAsync(s->bforce, 0, sizeof(float4) * (size_t)s->c.nb, st));
     }
-    int rc = enqueue_fluid_grid_and_density(s, st, method == 0);
+    int rc = enqueue_fluid_grid_and_lists(s, st);
     if (rc) return rc;
     float4 *vcur = s->velB;
     if (nf > 0) {
         PassCtx p = make_ctx(s);
         if (method == 0) {
-            // divergence-free solve (A5).  The loop is peeled: the P-pass of its first iteration ran
-            // inside k_density_alpha, the first C-pass and predicate follow here, further
-            // iterations (rare under the default tolerance) are the WHILE body.
+            // divergence-free solve (A5).  The loop is peeled: the P-pass of its first iteration runs
+            // inside k_density_alpha (which also sets the predicate), the first C-pass follows,
+            // further iterations (rare under the default tolerance) are the WHILE body.  The last
+            // C-pass adds dt g (A6) unless a viscosity kernel follows.
             rc = run_loop(s, graph_mode, &bc[LOOP_DIV],
-                [&](const LoopCtx &lc) -> int { return enqueue_solver_c<LIST>(s, lc, MODE_DIV, s->velB); },
-                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->velB); });
+                [&](const LoopCtx &lc) -> int {
+                    int r = enqueue_density(s, lc, true);
+                    if (r) return r;
+                    return enqueue_solver_c<LIST>(s, lc.st, TAIL_DIV, s->velB);
+                },
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->velB, 0); });
             if (rc) return rc;
             // non-pressure accelerations (A6 / A11)
             if (s->prm.viscosity_mode == 1) {
                 LAUNCH(s, (k_explicit_viscosity<LIST, false>), s->nblocks, kBlock, st, p, s->velB, s->velC);
                 vcur = s->velC;
-            } else {
-                LAUNCH(s, k_gravity, cdiv(nf, 256), 256, st, s->c, s->velB, s->velB);
-                if (s->prm.viscosity_mode == 2) {
-                    rc = run_loop(s, graph_mode, &bc[LOOP_CG],
-                        [&](const LoopCtx &lc) -> int {
-                            LAUNCH(s, (k_cg_apply<LIST, true>), s->nblocks, kBlock, lc.st, p, s->velB, s->cg_r, s->cg_p, s->partial, s->partial2);
-                            LAUNCH(s, k_cg_ctrl0, 1, kCtrlThreads, lc.st, s->partial, s->partial2, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
-                            return (int)SPH_OK;
-                        },
-                        [&](const LoopCtx &lc) -> int {
-                            LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, s->cg_p, s->cg_Ap, (float4 *)nullptr, s->partial, (float *)nullptr);
-                            LAUNCH(s, k_cg_ctrl1, 1, kCtrlThreads, lc.st, s->partial, s->nblocks, s->ctl);
-                            LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->velB, s->cg_r, s->partial2);
-                            LAUNCH(s, k_cg_ctrl2, 1, kCtrlThreads, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);
-                            LAUNCH(s, k_cg_direction, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_r, s->cg_p);
-                            return (int)SPH_OK;
-                        });
-                    if (rc) return rc;
-                }
+            } else if (s->prm.viscosity_mode == 2) {
+                rc = run_loop(s, graph_mode, &bc[LOOP_CG],
+                    [&](const LoopCtx &lc) -> int {
+                        LAUNCH(s, (k_cg_apply<LIST, true>), s->nblocks, kBlock, lc.st, p, s->velB, s->cg_r, s->cg_p, s->partial, s->partial2);
+                        LAUNCH(s, k_cg_ctrl0, 1, kCtrlThreads, lc.st, s->partial, s->partial2, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
+                        return (int)SPH_OK;
+                    },
+                    [&](const LoopCtx &lc) -> int {
+                        LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, s->cg_p, s->cg_Ap, (float4 *)nullptr, s->partial, (float *)nullptr);
+                        LAUNCH(s, k_cg_ctrl1, 1, kCtrlThreads, lc.st, s->partial, s->nblocks, s->ctl);
+                        LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->velB, s->cg_r, s->partial2);
+                        LAUNCH(s, k_cg_ctrl2, 1, kCtrlThreads, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);
+                        LAUNCH(s, k_cg_direction, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_r, s->cg_p);
+                        return (int)SPH_OK;
+                    });
+                if (rc) return rc;
             }
-            // constant-density solve (A7)
+            // constant-density solve (A7), peeled the same way; its last C-pass integrates (A9)
             rc = run_loop(s, graph_mode, &bc[LOOP_DENS],
-                [&](const LoopCtx &lc) -> int { LAUNCH(s, k_loop_init, 1, 1, lc.st, (int)LOOP_DENS, s->ctl, lc.h, lc.use_handle); return (int)SPH_OK; },
-                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur); });
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur, 1); },
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur, 0); });
             if (rc) return rc;
         } else {
-            // WCSPH (A10)
+            // WCSPH (A10): rho, EOS, [viscosity], one C-pass that also adds dt g and integrates
+            LoopCtx plain{ st, 0, 0 };
+            rc = enqueue_density(s, plain, false);
+            if (rc) return rc;
             LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->velB, s->posk);
             if (s->prm.viscosity_mode == 1) {
                 LAUNCH(s, (k_explicit_viscosity<LIST, true>), s->nblocks, kBlock, st, p, s->velB, s->velC);
                 vcur = s->velC;
-            } else {
-                LAUNCH(s, k_gravity, cdiv(nf, 256), 256, st, s->c, s->velB, s->velB);
             }
-            LAUNCH(s, k_solver_c<LIST>, s->nblocks, kBlock, st, p, s->posk, vcur);
-            if (dyn && s->ndyn > 0)
-                LAUNCH(s, k_boundary_force, cdiv(s->ndyn, kBlock), kBlock, st, s->c, s->dyn_idx, s->ndyn, s->borig_pos,
-                       s->posk, s->gf.cell_start, s->bforce);
+            rc = enqueue_solver_c<LIST>(s, st, TAIL_WCSPH, vcur);
+            if (rc) return rc;
         }
-        LAUNCH(s, k_integrate, cdiv(nf, 256), 256, st, s->c, s->posB, vcur, s->idB, s->posA, s->velA, s->idA,
-               &s->stats->vmax_bits, &s->stats->nan_count);
     }
     if (dyn && s->nbodies > 0)
         LAUNCH(s, k_rigid_step, s->nbodies, 256, st, s->c, s->bodies, s->prm.tank_min[0], s->prm.tank_min[1],
@@ -748,7 +756,8 @@ int sph_build_grid(SphSim *s)
         int rc = enqueue_boundary_grid(s, st);
         if (rc) return rc;
     }
-    int rc = enqueue_fluid_grid_and_density(s, st, false);
+    int rc = enqueue_fluid_grid_and_lists(s, st);
+    if (!rc) { LoopCtx plain{ st, 0, 0 }; rc = enqueue_density(s, plain, false); }
     if (rc) return rc;
     // leave the persistent store sorted as well (the next step's sort is then the identity)
     const size_t nf = (size_t)s->c.nf;
@@ -850,7 +859,11 @@ long long sph_launch_count(SphSim *s)
         // normally uses one method, so attribute them to the method that has run
         int m = s->graph_steps[0] > 0 ? 0 : 1;
         n += s->graph_steps[0] * s->fixed_nodes[0] + s->graph_steps[1] * s->fixed_nodes[1];
-        n += st.total_it_v * s->body_nodes[m][LOOP_DIV] + st.total_it_d * s->body_nodes[m][LOOP_DENS] +
+        // the divergence and density loops are peeled: their WHILE bodies run (iterations - 1) times per step
+        const long long steps = s->graph_steps[0] + s->graph_steps[1];
+        const long long body_v = st.total_it_v > steps ? st.total_it_v - steps : 0;
+        const long long body_d = st.total_it_d > steps ? st.total_it_d - steps : 0;
+        n += body_v * s->body_nodes[m][LOOP_DIV] + body_d * s->body_nodes[m][LOOP_DENS] +
              st.total_cg_iters * s->body_nodes[m][LOOP_CG];
     }
     return n;

@@ -50,6 +50,7 @@ struct DevControl {
     int it;                              // iteration counter of the running loop
     double cg_bb, cg_rr, cg_alpha, cg_beta;
     int cg_break;
+    unsigned long long acc;              // running P-pass: CTA counter (top 20 bits) | fixed-point error sum (A12)
 };
 
 // Statistics block in device memory; sph_read_stats copies it out and converts to SphStats.

@@ -15,6 +15,8 @@
 
 namespace sph {
 
+enum { MODE_DIV = 0, MODE_DENS = 1 };
+
 struct PassCtx {
     SimConst c;
     const float4 *pos;
@@ -359,6 +361,106 @@ k_build_lists(PassCtx p, ListCounters *__restrict__ lc, int rows)
 }
 
 // ---------------------------------------------------------------------------------------------
+// A12: device-side reductions and loop control.  Every P-pass reduces its error term on the
+// device; the LAST CTA of the launch to finish evaluates the loop predicate of Alg. 2
+// (R14: the error measured by this iteration's P-pass decides whether another
+// iteration follows its C-pass) and sets the CUDA-graph WHILE condition -- no host round trip and
+// no separate control launch (solver_tail below).  reduce_partials serves the CG dot products.  The C-pass that follows reads ctl->cont: the last C-pass of
+// a loop also does the work that follows the loop (gravity after the divergence solve,
+// integration after the density solve).
+__device__ __forceinline__ double reduce_partials(const float *__restrict__ partial, int n, double *sm)
+{
+    // fixed summation order (deterministic): float4 loads that bypass L1 (the partials were written
+    // by other SMs, possibly during this very launch), four chains per thread
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    const int st = blockDim.x, n4 = n >> 2;
+    const float4 *p4 = reinterpret_cast<const float4 *>(partial);
+    int k = threadIdx.x;
+    for (; k + 3 * st < n4; k += 4 * st) {
+        float4 a = __ldcg(p4 + k), b = __ldcg(p4 + k + st), c = __ldcg(p4 + k + 2 * st), d = __ldcg(p4 + k + 3 * st);
+        s0 += ((double)a.x + (double)a.y) + ((double)a.z + (double)a.w);
+        s1 += ((double)b.x + (double)b.y) + ((double)b.z + (double)b.w);
+        s2 += ((double)c.x + (double)c.y) + ((double)c.z + (double)c.w);
+        s3 += ((double)d.x + (double)d.y) + ((double)d.z + (double)d.w);
+    }
+    for (; k < n4; k += st) {
+        float4 a = __ldcg(p4 + k);
+        s0 += ((double)a.x + (double)a.y) + ((double)a.z + (double)a.w);
+    }
+    for (k = (n4 << 2) + threadIdx.x; k < n; k += st) s1 += (double)__ldcg(partial + k);
+    return block_sum((s0 + s1) + (s2 + s3), sm);
+}
+
+__device__ __forceinline__ void set_loop_condition(cudaGraphConditionalHandle h, int use_handle,
+                                                   DevControl *ctl, int cont)
+{
+    ctl->cont = cont;
+    if (use_handle) cudaGraphSetConditional(h, cont ? 1u : 0u);
+}
+
+struct LoopHandle { cudaGraphConditionalHandle h; int use_handle; };
+
+// thread 0 of the last CTA: predicate of the divergence (MODE_DIV) / density (MODE_DENS) loop.
+// err: the loop's error measure (R6); first: this P-pass opens the loop (iteration counter restarts at 1).
+template <int MODE>
+__device__ __forceinline__ void solver_ctrl_eval(double err, DevControl *ctl, DevStats *st, LoopHandle lh, bool first)
+{
+    const bool on = MODE == MODE_DIV ? (ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0)
+                                     : (ctl->forced_d != 0 && ctl->max_d > 0);
+    if (!on) {
+        // loop switched off: the peeled first iteration runs with kappa = 0 (a no-op on v)
+        if (MODE == MODE_DIV) { st->it_v = 0; st->err_v = 0.f; } else { st->it_d = 0; st->err_rho = 0.f; }
+        ctl->it = 0;
+        set_loop_condition(lh.h, lh.use_handle, ctl, 0);
+        return;
+    }
+    const int l = first ? 1 : ctl->it + 1;
+    ctl->it = l;
+    int cont;
+    if (MODE == MODE_DIV) {
+        int f = ctl->forced_v;
+        cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_v || l < ctl->min_v) && l < ctl->max_v);
+        st->it_v = l; st->err_v = (float)err;
+        if (f < 0 && !cont && err > (double)ctl->eta_v) st->max_iter_hit |= 1;
+    } else {
+        int f = ctl->forced_d;
+        cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_d || l < ctl->min_d) && l < ctl->max_d);
+        st->it_d = l; st->err_rho = (float)err;
+        if (f < 0 && !cont && err > (double)ctl->eta_d) st->max_iter_hit |= 2;
+    }
+    set_loop_condition(lh.h, lh.use_handle, ctl, cont);
+}
+
+// End of a P-pass kernel: `term` is this thread's error term (R_i or E_i >= 0).  All threads of the
+// CTA call it.  The CTA's sum (fixed shuffle order, fp32) is made dimensionless -- dt/rho0 * sum R_i
+// (R6: density change per step) or sum E_i / rho0 (R6) -- converted to 44-bit fixed point (2^-20
+// resolution) and added, together with a 1 in the CTA counter held in the top 20 bits, by ONE 64-bit
+// atomic: integer addition is associative, so the total is bit-identical whatever order the CTAs
+// arrive in, and the atomic's return value tells the last CTA that it is the last and what the
+// total is -- no fence, no partial array, no second pass.  Contributions are clamped so that the
+// 44-bit field cannot carry into the counter (a mean error above ~13 at 1.2M particles saturates).
+constexpr int kAccFracBits = 20, kAccSumBits = 44;
+
+template <int MODE>
+__device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevControl *ctl, DevStats *st,
+                                            LoopHandle lh, bool first)
+{
+    __shared__ float red[kBlock / 32];
+    float s = block_sum(term, red);
+    if (threadIdx.x != 0) return;
+    const double norm = MODE == MODE_DIV ? (double)c.dt / (double)c.rho0 : 1.0 / (double)c.rho0;
+    const unsigned long long cap = ((1ull << kAccSumBits) - 1ull) / (unsigned long long)gridDim.x;
+    double d = (double)s * norm * (double)(1u << kAccFracBits) + 0.5;
+    unsigned long long q = d > 0.0 ? (d < (double)cap ? (unsigned long long)d : cap) : 0ull;   // NaN -> 0
+    unsigned long long old = atomicAdd(&ctl->acc, (1ull << kAccSumBits) | q);
+    if ((old >> kAccSumBits) != (unsigned long long)(gridDim.x - 1)) return;
+    ctl->acc = 0ull;                                            // every CTA has arrived: reset for the next pass
+    unsigned long long total = (old & ((1ull << kAccSumBits) - 1ull)) + q;
+    double err = c.nf > 0 ? (double)total / (double)(1u << kAccFracBits) / (double)c.nf : 0.0;
+    solver_ctrl_eval<MODE>(err, ctl, st, lh, first);
+}
+
+// ---------------------------------------------------------------------------------------------
 // A4 second half: density (Eq. 4 + Eq. 12; self term included, R2) and the
 // DFSPH factor alpha_i = rho_i / (|S_i|^2 + T_i), S_i = sum_j m gradW_ij + sum_k Psi_k gradW_ik,
 // T_i = sum_j |m gradW_ij|^2 (R5, R7).
@@ -367,15 +469,12 @@ k_build_lists(PassCtx p, ListCounters *__restrict__ lc, int rows)
 // alpha_i that this very loop produces -- one full neighbour pass less per step.  It writes
 // posk[i] = (x_i, kappa^v_i / rho_i) (0 when the divergence solve is switched off) and the CTA
 // partial of R_i = max(D_i, 0).
-enum { MODE_DIV = 0, MODE_DENS = 1 };
-
 template <bool LIST, bool DIVP, bool DYN>
 __global__ void __launch_bounds__(kBlock)
 k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ bvel,
                 float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
-                const DevControl *__restrict__ ctl)
+                DevControl *ctl, DevStats *st, LoopHandle lh)
 {
-    __shared__ float red[kBlock / 32];
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -433,10 +532,7 @@ k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ 
             posk[i] = make_float4(xi.x, xi.y, xi.z, on ? kappa / rho : 0.f);
         }
     }
-    if (DIVP) {
-        float s = block_sum(term, red);
-        if (threadIdx.x == 0) partial[blockIdx.x] = s;
-    }
+    if (DIVP) solver_tail<MODE_DIV>(c, term, ctl, st, lh, true);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -450,9 +546,9 @@ k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ 
 template <bool LIST, int MODE, bool DYN>
 __global__ void __launch_bounds__(kBlock)
 k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__ bvel,
-           const float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial)
+           const float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
+           DevControl *ctl, DevStats *st, LoopHandle lh, int first)
 {
-    __shared__ float red[kBlock / 32];
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -484,55 +580,101 @@ k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__
         } else {
             term = fmaxf(fmaf(c.dt, D, rho), c.rho0) - c.rho0;
             kappa = a * term / (c.dt * c.dt);
+            // the P-pass that opens the density loop runs even when the loop is switched off
+            // (forced 0 iterations): kappa = 0 then, and its C-pass only integrates
+            if (first && !(ctl->forced_d != 0 && ctl->max_d > 0)) kappa = 0.f;
         }
         posk[i] = make_float4(xi.x, xi.y, xi.z, kappa / rho);
     }
-    float s = block_sum(term, red);
-    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+    solver_tail<MODE>(c, term, ctl, st, lh, first != 0);
 }
 
 // C-pass (A5 / A7 / A10): pressure-like velocity update (Eq. 7 + Eq. 13 with p/rho^2 == kappa/rho,
 // PAPER.md:123, 200):  v_i -= dt [ sum_j m (kr_i + kr_j) gradW_ij + sum_k Psi_k kr_i gradW_ik ].
-template <bool LIST>
+// The LAST C-pass of a loop (ctl->cont == 0, set by the P-pass before it) also does what follows the
+// loop, on the value it holds in registers:
+//   TAIL_DIV : v += dt g              (A6 without viscosity, Alg. 1 l.1-2; add_gravity)
+//   TAIL_DENS: x += dt v with the updated v (A9, symplectic Euler, Alg. 1 l.5-6); writes
+//              the persistent store (pos_out, vel_out, id_out) that the next step's sort reads and
+//              the step's v_max / non-finite counters
+//   TAIL_WCSPH: as TAIL_DENS, unconditionally (the WCSPH step has one C-pass).
+enum { TAIL_DIV = 0, TAIL_DENS = 1, TAIL_WCSPH = 2 };
+
+struct CTail {
+    const DevControl *ctl;
+    int add_gravity;
+    const int *id;
+    float4 *pos_out, *vel_out;
+    int *id_out;
+    unsigned *vmax_bits;
+    int *nan_count;
+};
+
+template <bool LIST, int TAIL>
 __global__ void __launch_bounds__(kBlock)
-k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel)
+k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel, CTail t)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= c.nf) return;
-    float4 xi = posk[i];
-    float kri = xi.w;
-    float fx = 0.f, fy = 0.f, fz = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-    for_each_neighbor<LIST, true, 1>(p, posk, posk, tbl, i, xi.x, xi.y, xi.z,
-        [&](int, float4 pj, float4, float dx, float dy, float dz, float d2) {
-            float s = (kri + pj.w) * pair_gradf(c, d2);
-            fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz);
-        },
-        [&](int, float4 pk, float dx, float dy, float dz, float d2) {
-            float s = pk.w * pair_gradf(c, d2);
-            bx = fmaf(s, dx, bx); by = fmaf(s, dy, by); bz = fmaf(s, dz, bz);
-        });
-    float4 v = vel[i];
-    float k = c.dt * c.grad_c;
-    v.x -= k * fmaf(c.m, fx, kri * bx);
-    v.y -= k * fmaf(c.m, fy, kri * by);
-    v.z -= k * fmaf(c.m, fz, kri * bz);
-    vel[i] = v;
+    const bool last = TAIL == TAIL_WCSPH || t.ctl->cont == 0;
+    float v2 = 0.f;
+    bool bad = false;
+    if (i < c.nf) {
+        float4 xi = posk[i];
+        float kri = xi.w;
+        float fx = 0.f, fy = 0.f, fz = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
+        for_each_neighbor<LIST, true, 1>(p, posk, posk, tbl, i, xi.x, xi.y, xi.z,
+            [&](int, float4 pj, float4, float dx, float dy, float dz, float d2) {
+                float s = (kri + pj.w) * pair_gradf(c, d2);
+                fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz);
+            },
+            [&](int, float4 pk, float dx, float dy, float dz, float d2) {
+                float s = pk.w * pair_gradf(c, d2);
+                bx = fmaf(s, dx, bx); by = fmaf(s, dy, by); bz = fmaf(s, dz, bz);
+            });
+        float4 v = vel[i];
+        if (TAIL == TAIL_WCSPH && t.add_gravity) {              // A10: v + dt g first, then the pressure term
+            v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
+        }
+        float k = c.dt * c.grad_c;
+        v.x -= k * fmaf(c.m, fx, kri * bx);
+        v.y -= k * fmaf(c.m, fy, kri * by);
+        v.z -= k * fmaf(c.m, fz, kri * bz);
+        if (TAIL == TAIL_DIV) {
+            if (last && t.add_gravity) {
+                v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
+            }
+            vel[i] = v;
+        } else {
+            vel[i] = v;
+            if (last) {
+                float4 x;
+                x.x = fmaf(c.dt, v.x, xi.x); x.y = fmaf(c.dt, v.y, xi.y); x.z = fmaf(c.dt, v.z, xi.z);
+                x.w = 0.f;
+                t.pos_out[i] = x;
+                t.vel_out[i] = make_float4(v.x, v.y, v.z, 0.f);
+                t.id_out[i] = t.id[i];
+                v2 = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
+                bad = !(isfinite(x.x) && isfinite(x.y) && isfinite(x.z) && isfinite(v2));
+                if (bad) v2 = 0.f;
+            }
+        }
+    }
+    if (TAIL != TAIL_DIV && last) {
+        v2 = warp_max(v2);
+        unsigned b = __ballot_sync(0xffffffffu, bad);
+        if ((threadIdx.x & 31) == 0) {
+            unsigned vb = __float_as_uint(sqrtf(v2));           // non-negative floats order like their bits
+            if (vb > *(volatile unsigned *)t.vmax_bits) atomicMax(t.vmax_bits, vb);   // guarded: same-address atomics serialise
+            if (b) atomicAdd(t.nan_count, __popc(b));
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
 // A6, Alg. 1 l.1-2: v* = v + dt (g + a_visc).
-// mode 0 / 2: gravity only (elementwise; in place is fine).
-__global__ void __launch_bounds__(256)
-k_gravity(SimConst c, const float4 *__restrict__ vin, float4 *__restrict__ vout)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= c.nf) return;
-    float4 v = vin[i];
-    v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
-    vout[i] = v;
-}
+// mode 0 / 2: gravity only -- folded into the last C-pass of the divergence solve (TAIL_DIV above).
 
 // mode 1: explicit viscosity, Eq. 15 (R4, R16, R22):
 //   a_i = nu 2(d+2) sum_j (m / rho_j) (v_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij, fluid-fluid only.
@@ -666,61 +808,6 @@ k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const float4 *__restrict
     posk[i] = make_float4(x.x, x.y, x.z, pr / (rt * rt));
 }
 
-// ---------------------------------------------------------------------------------------------
-// A9: symplectic Euler (Alg. 1 l.5-6): x += dt v with the already updated v.
-// Writes the persistent store (pos_out, vel_out, id_out) that the next step's sort reads, and the
-// step's v_max / non-finite counters.
-__global__ void __launch_bounds__(256)
-k_integrate(SimConst c, const float4 *__restrict__ pos, const float4 *__restrict__ vel,
-            const int *__restrict__ id, float4 *__restrict__ pos_out, float4 *__restrict__ vel_out,
-            int *__restrict__ id_out, unsigned *__restrict__ vmax_bits, int *__restrict__ nan_count)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    float v2 = 0.f;
-    bool bad = false;
-    if (i < c.nf) {
-        float4 x = pos[i], v = vel[i];
-        x.x = fmaf(c.dt, v.x, x.x); x.y = fmaf(c.dt, v.y, x.y); x.z = fmaf(c.dt, v.z, x.z);
-        x.w = 0.f;
-        pos_out[i] = x;
-        vel_out[i] = make_float4(v.x, v.y, v.z, 0.f);
-        id_out[i] = id[i];
-        v2 = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
-        bad = !(isfinite(x.x) && isfinite(x.y) && isfinite(x.z) && isfinite(v2));
-        if (bad) v2 = 0.f;
-    }
-    v2 = warp_max(v2);
-    unsigned b = __ballot_sync(0xffffffffu, bad);
-    if ((threadIdx.x & 31) == 0) {
-        unsigned vb = __float_as_uint(sqrtf(v2));           // non-negative floats order like their bits
-        if (vb > *(volatile unsigned *)vmax_bits) atomicMax(vmax_bits, vb);   // guarded: same-address atomics serialise
-        if (b) atomicAdd(nan_count, __popc(b));
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// A12: loop control.  One CTA sums the per-CTA partials in a fixed order (fp64), evaluates the
-// loop predicate of Alg. 2 (R14: the error measured by this iteration's P-pass
-// is tested after its C-pass) and sets the CUDA-graph WHILE condition -- no host round trip.
-__device__ __forceinline__ double reduce_partials(const float *__restrict__ partial, int n, double *sm)
-{
-    // fixed summation order (deterministic): four independent strided chains per thread
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-    const int st = blockDim.x;
-    int k = threadIdx.x;
-    for (; k + 3 * st < n; k += 4 * st) {
-        float a = partial[k], b = partial[k + st], c = partial[k + 2 * st], d = partial[k + 3 * st];
-        s0 += (double)a; s1 += (double)b; s2 += (double)c; s3 += (double)d;
-    }
-    for (; k < n; k += st) s0 += (double)partial[k];
-    return block_sum((s0 + s1) + (s2 + s3), sm);
-}
-
-__device__ __forceinline__ void set_loop_condition(cudaGraphConditionalHandle h, int use_handle,
-                                                   DevControl *ctl, int cont)
-{
-    ctl->cont = cont;
-    if (use_handle) cudaGraphSetConditional(h, cont ? 1u : 0u);
-}
+// A9 (symplectic Euler) is the tail of the last C-pass: see k_solver_c, TAIL_DENS / TAIL_WCSPH.
 
 }  // namespace sph

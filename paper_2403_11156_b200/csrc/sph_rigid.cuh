@@ -297,49 +297,6 @@ __global__ void k_step_end(DevStats *st)
     st->total_it_v += st->it_v; st->total_it_d += st->it_d; st->total_cg += st->cg_iters;
 }
 
-// before a solver loop: reset the counter and decide whether the body runs at all
-__global__ void k_loop_init(int kind, DevControl *ctl, cudaGraphConditionalHandle h, int use_handle)
-{
-    ctl->it = 0;
-    int cont;
-    if (kind == LOOP_DIV) cont = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;   // (unused: the divergence loop is peeled)
-    else cont = ctl->forced_d != 0 && ctl->max_d > 0;
-    set_loop_condition(h, use_handle, ctl, cont);
-}
-
-template <int MODE>
-__global__ void __launch_bounds__(kCtrlThreads)
-k_solver_ctrl(SimConst c, const float *__restrict__ partial, int nparts, DevControl *ctl,
-              DevStats *st, cudaGraphConditionalHandle h, int use_handle)
-{
-    __shared__ double sm[kCtrlThreads / 32];
-    double sum = reduce_partials(partial, nparts, sm);
-    if (threadIdx.x != 0) return;
-    double mean = c.nf > 0 ? sum / (double)c.nf : 0.0;
-    int cont;
-    if (MODE == MODE_DIV && !(ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0)) {
-        // divergence solve switched off: the peeled first iteration ran with kappa^v = 0 (a no-op)
-        st->it_v = 0; st->err_v = 0.f;
-        set_loop_condition(h, use_handle, ctl, 0);
-        return;
-    }
-    int l = ++ctl->it;
-    if (MODE == MODE_DIV) {
-        double err = (double)c.dt / (double)c.rho0 * mean;     // R6: density change per step
-        int f = ctl->forced_v;
-        cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_v || l < ctl->min_v) && l < ctl->max_v);
-        st->it_v = l; st->err_v = (float)err;
-        if (f < 0 && !cont && err > (double)ctl->eta_v) st->max_iter_hit |= 1;
-    } else {
-        double err = mean / (double)c.rho0;                    // R6: mean(rho* - rho0)/rho0
-        int f = ctl->forced_d;
-        cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_d || l < ctl->min_d) && l < ctl->max_d);
-        st->it_d = l; st->err_rho = (float)err;
-        if (f < 0 && !cont && err > (double)ctl->eta_d) st->max_iter_hit |= 2;
-    }
-    set_loop_condition(h, use_handle, ctl, cont);
-}
-
 // CG start: |b|^2, |r0|^2, first predicate (R23: stop when |r| <= tol |b| or max iterations)
 __global__ void __launch_bounds__(kCtrlThreads)
 k_cg_ctrl0(const float *__restrict__ pbb, const float *__restrict__ prr, int nparts, DevControl *ctl,
