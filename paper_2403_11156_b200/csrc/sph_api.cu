@@ -52,7 +52,8 @@ struct SphSim {
     int nblocks = 0;                // CTAs of the per-particle kernels (= number of partials)
     size_t cs_len = 0;              // ncells + 1 rounded up to 4
     // fluid store
-    float4 *posA = nullptr, *velA = nullptr, *posB = nullptr, *velB = nullptr, *velC = nullptr, *posk = nullptr;
+    float4 *posA = nullptr, *velA = nullptr, *posB = nullptr, *posk = nullptr;
+    PV *pvB = nullptr, *pvC = nullptr;   // { pos | vel, rho } records of the passes; pvC: output of explicit viscosity
     int *idA = nullptr, *idB = nullptr;
     float *alpha = nullptr;
     GridBufs gf, gb;
@@ -197,8 +198,8 @@ size_t layout(SphSim &s, void *base)
     s.ctl = w.take<DevControl>(1);
     s.stats = w.take<DevStats>(1);
     s.posA = w.take<float4>(nf1); s.velA = w.take<float4>(nf1); s.idA = w.take<int>(nf1);
-    s.posB = w.take<float4>(nf1 + kPosPad); s.velB = w.take<float4>(nf1); s.idB = w.take<int>(nf1);
-    s.velC = s.prm.viscosity_mode == 1 ? w.take<float4>(nf1) : nullptr;
+    s.posB = w.take<float4>(nf1 + kPosPad); s.pvB = w.take<PV>(nf1); s.idB = w.take<int>(nf1);
+    s.pvC = s.prm.viscosity_mode == 1 ? w.take<PV>(nf1) : nullptr;
     s.posk = w.take<float4>(nf1);
     s.alpha = w.take<float>(nf1);
     s.gf.n = (int)nf;
@@ -235,7 +236,7 @@ size_t layout(SphSim &s, void *base)
 // ------------------------------------------------------------------------------------------
 // A1-A3 on one particle set: keys + histogram, scan, scatter, canonical reorder.
 int enqueue_grid(SphSim *s, cudaStream_t st, GridBufs &g, const float4 *a_in, const float4 *b_in,
-                 const int *id_in, float4 *a_out, float4 *b_out, int *id_out, int *oob)
+                 const int *id_in, float4 *a_out, float4 *b_out, int *id_out, int *oob, bool fluid)
 {
     CUDA_TRY(s, cudaMemsetAsync(g.cell_start, 0, s->cs_len * sizeof(int), st));
     if (g.n > 0)
@@ -246,8 +247,10 @@ int enqueue_grid(SphSim *s, cudaStream_t st, GridBufs &g, const float4 *a_in, co
     LAUNCH(s, k_scan_apply, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
     if (g.n > 0) {
         LAUNCH(s, k_scatter_slots, cdiv(g.n, 256), 256, st, g.key, g.off, g.cell_start, g.n, g.slot);
-        LAUNCH(s, k_reorder, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
-               a_out, b_out, id_out);
+        if (fluid) LAUNCH(s, k_reorder<true>, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
+                          a_out, b_out, id_out);
+        else       LAUNCH(s, k_reorder<false>, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
+                          a_out, b_out, id_out);
     }
     return SPH_OK;
 }
@@ -264,7 +267,7 @@ PassCtx make_ctx(const SphSim *s)
 
 int enqueue_boundary_grid(SphSim *s, cudaStream_t st)
 {
-    return enqueue_grid(s, st, s->gb, s->borig_pos, s->borig_vel, nullptr, s->bpos_s, s->bvel_s, s->bid_s, nullptr);
+    return enqueue_grid(s, st, s->gb, s->borig_pos, s->borig_vel, nullptr, s->bpos_s, s->bvel_s, s->bid_s, nullptr, false);
 }
 
 // Solver loops.  graph mode: a conditional WHILE node whose body is captured on the helper
@@ -278,7 +281,7 @@ struct LoopCtx {
 // A1-A3 on the fluid, then the neighbour lists (A4 first half).
 int enqueue_fluid_grid_and_lists(SphSim *s, cudaStream_t st)
 {
-    int rc = enqueue_grid(s, st, s->gf, s->posA, s->velA, s->idA, s->posB, s->velB, s->idB, &s->stats->oob);
+    int rc = enqueue_grid(s, st, s->gf, s->posA, s->velA, s->idA, s->posB, reinterpret_cast<float4 *>(s->pvB), s->idB, &s->stats->oob, true);
     if (rc) return rc;
     if (s->c.nf > 0) {
         PassCtx p = make_ctx(s);
@@ -303,7 +306,7 @@ int enqueue_density(SphSim *s, const LoopCtx &lc, bool divp)
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
     LoopHandle lh{ lc.h, lc.use_handle };
-#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->velB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl, s->stats, lh)
+#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->pvB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl, s->stats, lh)
     if (s->prm.use_neighbor_list) {
         if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
     } else {
@@ -373,7 +376,7 @@ int run_loop(SphSim *s, bool graph_mode, long long *body_counter, Init init, Bod
 
 // P-pass of one solver iteration (its last CTA evaluates the loop predicate, A12)
 template <bool LIST>
-int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, float4 *vel, int first)
+int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, PV *vel, int first)
 {
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
@@ -387,7 +390,7 @@ int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, float4 *vel, int fi
 
 // C-pass (with the tail work of the loop's last iteration) and the Eq. 14 reactions
 template <bool LIST>
-int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, float4 *vel)
+int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, PV *vel)
 {
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
@@ -406,7 +409,7 @@ int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, float4 *vel)
 }
 
 template <bool LIST>
-int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, float4 *vel, int first)
+int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, PV *vel, int first)
 {
     int rc = enqueue_solver_p<LIST>(s, lc, mode, vel, first);
     if (rc) return rc;
@@ -428,7 +431,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
     }
     int rc = enqueue_fluid_grid_and_lists(s, st);
     if (rc) return rc;
-    float4 *vcur = s->velB;
+    PV *vcur = s->pvB;
     if (nf > 0) {
         PassCtx p = make_ctx(s);
         if (method == 0) {
@@ -440,25 +443,25 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
                 [&](const LoopCtx &lc) -> int {
                     int r = enqueue_density(s, lc, true);
                     if (r) return r;
-                    return enqueue_solver_c<LIST>(s, lc.st, TAIL_DIV, s->velB);
+                    return enqueue_solver_c<LIST>(s, lc.st, TAIL_DIV, s->pvB);
                 },
-                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->velB, 0); });
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->pvB, 0); });
             if (rc) return rc;
             // non-pressure accelerations (A6 / A11)
             if (s->prm.viscosity_mode == 1) {
-                LAUNCH(s, (k_explicit_viscosity<LIST, false>), s->nblocks, kBlock, st, p, s->velB, s->velC);
-                vcur = s->velC;
+                LAUNCH(s, (k_explicit_viscosity<LIST, false>), s->nblocks, kBlock, st, p, s->pvB, s->pvC);
+                vcur = s->pvC;
             } else if (s->prm.viscosity_mode == 2) {
                 rc = run_loop(s, graph_mode, &bc[LOOP_CG],
                     [&](const LoopCtx &lc) -> int {
-                        LAUNCH(s, (k_cg_apply<LIST, true>), s->nblocks, kBlock, lc.st, p, s->velB, s->cg_r, s->cg_p, s->partial, s->partial2);
+                        LAUNCH(s, (k_cg_apply<LIST, true>), s->nblocks, kBlock, lc.st, p, reinterpret_cast<const float4 *>(s->pvB), s->cg_r, s->cg_p, s->partial, s->partial2);
                         LAUNCH(s, k_cg_ctrl0, 1, kCtrlThreads, lc.st, s->partial, s->partial2, s->nblocks, s->ctl, s->stats, lc.h, lc.use_handle);
                         return (int)SPH_OK;
                     },
                     [&](const LoopCtx &lc) -> int {
                         LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, s->cg_p, s->cg_Ap, (float4 *)nullptr, s->partial, (float *)nullptr);
                         LAUNCH(s, k_cg_ctrl1, 1, kCtrlThreads, lc.st, s->partial, s->nblocks, s->ctl);
-                        LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->velB, s->cg_r, s->partial2);
+                        LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->pvB, s->cg_r, s->partial2);
                         LAUNCH(s, k_cg_ctrl2, 1, kCtrlThreads, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);
                         LAUNCH(s, k_cg_direction, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_r, s->cg_p);
                         return (int)SPH_OK;
@@ -475,10 +478,10 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
             LoopCtx plain{ st, 0, 0 };
             rc = enqueue_density(s, plain, false);
             if (rc) return rc;
-            LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->velB, s->posk);
+            LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->pvB, s->posk);
             if (s->prm.viscosity_mode == 1) {
-                LAUNCH(s, (k_explicit_viscosity<LIST, true>), s->nblocks, kBlock, st, p, s->velB, s->velC);
-                vcur = s->velC;
+                LAUNCH(s, (k_explicit_viscosity<LIST, true>), s->nblocks, kBlock, st, p, s->pvB, s->pvC);
+                vcur = s->pvC;
             }
             rc = enqueue_solver_c<LIST>(s, st, TAIL_WCSPH, vcur);
             if (rc) return rc;
@@ -574,9 +577,9 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
     switch (field) {
     case SPH_FIELD_POS: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->posA, s->idA, nf, (float *)out); break;
     case SPH_FIELD_VEL: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->velA, s->idA, nf, (float *)out); break;
-    case SPH_FIELD_DENSITY: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->velB, s->idB, nf, (float *)out); break;
+    case SPH_FIELD_DENSITY: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, &s->pvB->v, s->idB, nf, (float *)out, 2); break;
     case SPH_FIELD_ALPHA: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->alpha, s->idB, nf, (float *)out); break;
-    case SPH_FIELD_KAPPA_OVER_RHO: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posk, s->idB, nf, (float *)out); break;
+    case SPH_FIELD_KAPPA_OVER_RHO: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posk, s->idB, nf, (float *)out, 1); break;
     case SPH_FIELD_CELL_START:
         CUDA_TRY(s, cudaMemcpyAsync(out, s->gf.cell_start, bytes, cudaMemcpyDeviceToDevice, st)); break;
     case SPH_FIELD_BOUNDARY_CELL_START:
@@ -594,7 +597,7 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
         LAUNCH(s, k_export_neighbors, cdiv((long long)nf * s->c.kb, 256), 256, st, s->nl_b, s->ncount, 16, s->idB, s->bid_s, nf, s->c.kb, (int *)out); break;
     case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->borig_pos, (const int *)nullptr, nb, (float *)out); break;
     case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->borig_vel, (const int *)nullptr, nb, (float *)out); break;
-    case SPH_FIELD_BOUNDARY_PSI: LAUNCH(s, k_export_w, cdiv(nb, 256), 256, st, s->borig_pos, (const int *)nullptr, nb, (float *)out); break;
+    case SPH_FIELD_BOUNDARY_PSI: LAUNCH(s, k_export_w, cdiv(nb, 256), 256, st, s->borig_pos, (const int *)nullptr, nb, (float *)out, 1); break;
     case SPH_FIELD_BOUNDARY_FORCE: LAUNCH(s, k_export_vec3, cdiv(nb, 256), 256, st, s->bforce, (const int *)nullptr, nb, (float *)out); break;
     case SPH_FIELD_RIGID_BODIES:
         CUDA_TRY(s, cudaMemcpyAsync(out, s->bodies, bytes, cudaMemcpyDeviceToDevice, st)); break;
@@ -763,7 +766,7 @@ int sph_build_grid(SphSim *s)
     const size_t nf = (size_t)s->c.nf;
     if (nf > 0) {
         CUDA_TRY(s, cudaMemcpyAsync(s->posA, s->posB, nf * sizeof(float4), cudaMemcpyDeviceToDevice, st));
-        CUDA_TRY(s, cudaMemcpyAsync(s->velA, s->velB, nf * sizeof(float4), cudaMemcpyDeviceToDevice, st));
+        CUDA_TRY(s, cudaMemcpy2DAsync(s->velA, sizeof(float4), &s->pvB->v, sizeof(PV), sizeof(float4), nf, cudaMemcpyDeviceToDevice, st));
         CUDA_TRY(s, cudaMemcpyAsync(s->idA, s->idB, nf * sizeof(int), cudaMemcpyDeviceToDevice, st));
         // posk mirrors the positions with kappa/rho = 0 until a solver pass writes it
         CUDA_TRY(s, cudaMemcpyAsync(s->posk, s->posA, nf * sizeof(float4), cudaMemcpyDeviceToDevice, st));

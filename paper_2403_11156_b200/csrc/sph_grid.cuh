@@ -164,8 +164,10 @@ k_scatter_slots(const int *__restrict__ key, const int *__restrict__ off,
 // A3 second half: canonical order inside a cell = ascending source index (= order of the
 // previous sorted store, R12: makes the run bit-reproducible although the histogram atomics are
 // not), then gather of every persistent field into sorted order.
-// For the fluid store: a = pos(x,y,z,-), b = vel(vx,vy,vz,-), ids carried.
+// For the fluid store (FLUID): a = pos(x,y,z,-), b = vel(vx,vy,vz,-), ids carried; a_out = packed
+// positions, b_out = { pos | vel } records.
 // For the boundary store: a = (x,y,z,psi), b = (vx,vy,vz,-), ids = original boundary index.
+template <bool FLUID>
 __global__ void __launch_bounds__(256)
 k_reorder(const int *__restrict__ slot_src, const int *__restrict__ key,
           const int *__restrict__ cell_start, int n,
@@ -185,8 +187,13 @@ k_reorder(const int *__restrict__ slot_src, const int *__restrict__ key,
         for (int t = cs; t < ce; ++t) rank += (slot_src[t] < src) ? 1 : 0;
     }
     int dst = cs + rank;
-    a_out[dst] = a_in[src];
-    if (b_in != nullptr) b_out[dst] = b_in[src];
+    float4 a = a_in[src];
+    a_out[dst] = a;
+    if (FLUID) {
+        // b_out is the 32-byte record array { pos | vel } of the passes (PV in sph_passes.cuh)
+        b_out[2 * dst] = a;
+        b_out[2 * dst + 1] = b_in[src];
+    } else if (b_in != nullptr) b_out[dst] = b_in[src];
     id_out[dst] = id_in != nullptr ? id_in[src] : src;
 }
 

@@ -3,7 +3,13 @@
 //
 // Store layout (all fp32, sorted cell order, one thread per fluid particle):
 //   pos [nf] float4  x, y, z, -
-//   vel [nf] float4  vx, vy, vz, rho        (rho_i rides in .w: the viscosity sums need rho_j)
+//   pv  [nf] PV      32-byte record { x, y, z, - | vx, vy, vz, rho }: the passes that need position
+//                    AND velocity of a neighbour (A4 with the fused divergence P-pass, every P-pass,
+//                    viscosity) fetch both with ONE 256-bit gather (LDG.E.256, sm_100) -- the list
+//                    passes are bound by L1 gather wavefronts, and one 32-byte sector per neighbour
+//                    costs fewer of them than two 16-byte gathers from two arrays.  rho_i rides in
+//                    v.w: the viscosity sums need rho_j.  pos stays as a packed copy: the list
+//                    builder reads TWO candidates per 256-bit load from it.
 //   posk[nf] float4  x, y, z, kappa_i/rho_i (written by every P-pass, gathered by the C-pass:
 //                                            one 16-byte gather per neighbour instead of two)
 //   bpos[nb] float4  x, y, z, Psi           bvel[nb] float4 vx, vy, vz, -
@@ -16,6 +22,17 @@
 namespace sph {
 
 enum { MODE_DIV = 0, MODE_DENS = 1 };
+
+struct __align__(32) PV { float4 x, v; };   // position (x, y, z, -) | velocity (vx, vy, vz, rho)
+
+// 32 bytes (aligned) through the read-only path with one instruction
+__device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b)
+{
+    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+        : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
+        : "l"(p));
+}
+
 
 struct PassCtx {
     SimConst c;
@@ -100,7 +117,8 @@ __device__ __forceinline__ void fill_run_table(const Geom &g, const int *__restr
 // Visit every neighbour of fluid particle i (sorted index), fluid first then boundary, both in
 // ascending sorted index:
 //   ff(j, qj, q2j, dx, dy, dz, d2) for fluid j != i with d2 < h2,  fb(k, pk, dx, dy, dz, d2) for boundary k;
-//   d = x_i - x_j in fp32, d2 as in reading R10; qj = src[j], q2j = src2[j] (NSRC == 2, else qj).
+//   d = x_i - x_j in fp32, d2 as in reading R10; qj = src[j], q2j = src2[j] (NSRC == 2, else qj);
+//   NSRC == 3: src points at PV records, (qj, q2j) = (pv[j].x, pv[j].v) from one 256-bit load.
 // LIST = true : gather through the per-step list (predicate was evaluated when it was built).  The
 //   list words of the next stage are requested before the gathers of the current one are consumed,
 //   and all gathers of a stage are issued before their arithmetic: the pass is bound by memory
@@ -115,7 +133,7 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
 {
     const CellOf cell = cell_of(p.c.g, xi, yi, zi);
     if (LIST) {
-        constexpr int PB = NSRC == 2 ? SPH_PAIRS2 : SPH_PAIRS1;
+        constexpr int PB = NSRC >= 2 ? SPH_PAIRS2 : SPH_PAIRS1;
         const int packed = p.ncount[i];
         const int cf = packed & 0xffff, cb = (packed >> 16) & 0xffff;
         int *tbl = tbl_base + threadIdx.x;
@@ -131,7 +149,7 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
 #pragma unroll
             for (int t = 0; t < PB; ++t) nxt[t] = pb + PB + t < npair ? __ldg(lp + (pb + PB + t) * 32) : 0u;
             int jj[2 * PB];
-            float4 q[2 * PB], q2[NSRC == 2 ? 2 * PB : 1];
+            float4 q[2 * PB], q2[NSRC >= 2 ? 2 * PB : 1];
 #pragma unroll
             for (int u = 0; u < 2 * PB; ++u) {
                 const bool valid = 2 * pb + u < cf;
@@ -139,14 +157,17 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
                 e = valid ? e : 0u;                       // the unwritten half of an odd tail pair is garbage
                 int j = tbl[(e >> kOffBits) * kBlock] + (int)(e & kOffMask);
                 jj[u] = valid ? j : i;
-                q[u] = __ldg(src + jj[u]);
-                if (NSRC == 2) q2[u] = __ldg(src2 + jj[u]);
+                if (NSRC == 3) ldg256(src + 2 * jj[u], q[u], q2[u]);
+                else {
+                    q[u] = __ldg(src + jj[u]);
+                    if (NSRC == 2) q2[u] = __ldg(src2 + jj[u]);
+                }
             }
 #pragma unroll
             for (int u = 0; u < 2 * PB; ++u) {
                 if (2 * pb + u < cf) {
                     float dx = __fsub_rn(xi, q[u].x), dy = __fsub_rn(yi, q[u].y), dz = __fsub_rn(zi, q[u].z);
-                    ff(jj[u], q[u], NSRC == 2 ? q2[u] : q[u], dx, dy, dz, dist2_r10(dx, dy, dz));
+                    ff(jj[u], q[u], NSRC >= 2 ? q2[u] : q[u], dx, dy, dz, dist2_r10(dx, dy, dz));
                 }
             }
 #pragma unroll
@@ -165,10 +186,11 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
     } else {
         const float h2 = p.c.h2;
         for_each_candidate(p.c.g, p.fcs, cell, [&](int j, int, int) {
-            float4 q = __ldg(src + j);
+            float4 q, q2;
+            if (NSRC == 3) ldg256(src + 2 * j, q, q2); else q = __ldg(src + j);
             float dx = __fsub_rn(xi, q.x), dy = __fsub_rn(yi, q.y), dz = __fsub_rn(zi, q.z);
             float d2 = dist2_r10(dx, dy, dz);
-            if (d2 < h2 && j != i) ff(j, q, NSRC == 2 ? __ldg(src2 + j) : q, dx, dy, dz, d2);
+            if (d2 < h2 && j != i) ff(j, q, NSRC == 3 ? q2 : (NSRC == 2 ? __ldg(src2 + j) : q), dx, dy, dz, d2);
         });
         if (WITH_B && p.c.nb > 0) {
             for_each_candidate(p.c.g, p.bcs, cell, [&](int j, int, int) {
@@ -205,16 +227,6 @@ __device__ __forceinline__ float pair_gradf(const SimConst &c, float d2)
 constexpr int kPosPad = 4;         // float4 elements readable past pos[nf - 1]
 constexpr int kStageExtra = 32;    // staging rows beyond kf (a run longer than this takes the guarded loop)
 constexpr int kMaxListCap = 768;   // (kMaxListCap + kStageExtra) * 64 B * 4 warps <= 227 KB of shared memory
-
-__device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b)
-{
-#ifdef SPH_NO_LDG256
-    a = __ldg(p); b = __ldg(p + 1); return;
-#endif
-    asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-        : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
-        : "l"(p));
-}
 
 __device__ __forceinline__ void sts_u16(uint32_t addr, int v)
 {
@@ -471,7 +483,7 @@ __device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevCo
 // partial of R_i = max(D_i, 0).
 template <bool LIST, bool DIVP, bool DYN>
 __global__ void __launch_bounds__(kBlock)
-k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ bvel,
+k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
                 float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
                 DevControl *ctl, DevStats *st, LoopHandle lh)
 {
@@ -481,11 +493,11 @@ k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ 
     float term = 0.f;
     if (i < c.nf) {
         float4 xi = p.pos[i];
-        float4 vi = vel[i];
+        float4 vi = pv[i].v;
         float sw = 0.f, sx = 0.f, sy = 0.f, sz = 0.f, t2 = 0.f;    // fluid: sum w, sum gf d, sum gf^2 d2
         float bw = 0.f, bx = 0.f, by = 0.f, bz = 0.f;              // boundary, Psi-weighted
         float df = 0.f, db = 0.f;                                  // density rate (DIVP)
-        for_each_neighbor<LIST, true, DIVP ? 2 : 1>(p, p.pos, vel, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, true, DIVP ? 3 : 1>(p, DIVP ? reinterpret_cast<const float4 *>(pv) : p.pos, nullptr, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
                 float r, rinv;
                 r_and_rinv(d2, r, rinv);
@@ -522,7 +534,7 @@ k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ 
         float den = fmaf(Sx, Sx, fmaf(Sy, Sy, fmaf(Sz, Sz, T)));
         float a = den > 1e-6f ? rho / den : 0.0f;
         alpha[i] = a;
-        vel[i].w = rho;   // 4-byte store: concurrent gathers of vel[i] by other threads use xyz only
+        pv[i].v.w = rho;  // 4-byte store: concurrent gathers of pv[i] by other threads use xyz only
         if (DIVP) {
             // Eq. 10 source (R15): R_i = max(D_i, 0), kappa^v_i = alpha_i R_i / dt
             bool on = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;
@@ -545,7 +557,7 @@ k_density_alpha(PassCtx p, float4 *__restrict__ vel, const float4 *__restrict__ 
 
 template <bool LIST, int MODE, bool DYN>
 __global__ void __launch_bounds__(kBlock)
-k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__ bvel,
+k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel,
            const float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
            DevControl *ctl, DevStats *st, LoopHandle lh, int first)
 {
@@ -554,10 +566,10 @@ k_solver_p(PassCtx p, const float4 *__restrict__ vel, const float4 *__restrict__
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     float term = 0.f;
     if (i < c.nf) {
-        float4 xi = p.pos[i];
-        float4 vi = vel[i];
+        float4 xi, vi;
+        ldg256(reinterpret_cast<const float4 *>(pv + i), xi, vi);
         float df = 0.f, db = 0.f;
-        for_each_neighbor<LIST, true, 2>(p, p.pos, vel, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, true, 3>(p, reinterpret_cast<const float4 *>(pv), nullptr, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
                 float gf = pair_gradf(c, d2);
                 float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
@@ -612,7 +624,7 @@ struct CTail {
 
 template <bool LIST, int TAIL>
 __global__ void __launch_bounds__(kBlock)
-k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel, CTail t)
+k_solver_c(PassCtx p, const float4 *__restrict__ posk, PV *__restrict__ pv, CTail t)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
@@ -633,7 +645,7 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel,
                 float s = pk.w * pair_gradf(c, d2);
                 bx = fmaf(s, dx, bx); by = fmaf(s, dy, by); bz = fmaf(s, dz, bz);
             });
-        float4 v = vel[i];
+        float4 v = pv[i].v;
         if (TAIL == TAIL_WCSPH && t.add_gravity) {              // A10: v + dt g first, then the pressure term
             v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
         }
@@ -645,9 +657,9 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel,
             if (last && t.add_gravity) {
                 v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
             }
-            vel[i] = v;
+            pv[i].v = v;
         } else {
-            vel[i] = v;
+            pv[i].v = v;
             if (last) {
                 float4 x;
                 x.x = fmaf(c.dt, v.x, xi.x); x.y = fmaf(c.dt, v.y, xi.y); x.z = fmaf(c.dt, v.z, xi.z);
@@ -678,20 +690,20 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, float4 *__restrict__ vel,
 
 // mode 1: explicit viscosity, Eq. 15 (R4, R16, R22):
 //   a_i = nu 2(d+2) sum_j (m / rho_j) (v_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij, fluid-fluid only.
-// rho_j is vel[j].w; CLAMP = true (WCSPH, R17) uses rho~_j = max(rho_j, rho0).  Reads vin, writes
-// vout != vin.
+// rho_j is pv[j].v.w; CLAMP = true (WCSPH, R17) uses rho~_j = max(rho_j, rho0).  Reads the records vin,
+// writes the records vout != vin (position copied).
 template <bool LIST, bool CLAMP>
 __global__ void __launch_bounds__(kBlock)
-k_explicit_viscosity(PassCtx p, const float4 *__restrict__ vin, float4 *__restrict__ vout)
+k_explicit_viscosity(PassCtx p, const PV *__restrict__ vin, PV *__restrict__ vout)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.nf) return;
-    float4 xi = p.pos[i];
-    float4 vi = vin[i];
+    float4 xi, vi;
+    ldg256(reinterpret_cast<const float4 *>(vin + i), xi, vi);
     float ax = 0.f, ay = 0.f, az = 0.f;
-    for_each_neighbor<LIST, false, 2>(p, p.pos, vin, tbl, i, xi.x, xi.y, xi.z,
+    for_each_neighbor<LIST, false, 3>(p, reinterpret_cast<const float4 *>(vin), nullptr, tbl, i, xi.x, xi.y, xi.z,
         [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
             float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
             float rj = CLAMP ? fmaxf(vj.w, c.rho0) : vj.w;
@@ -703,19 +715,20 @@ k_explicit_viscosity(PassCtx p, const float4 *__restrict__ vin, float4 *__restri
     vi.x += fmaf(c.dt, c.gx, k * ax);
     vi.y += fmaf(c.dt, c.gy, k * ay);
     vi.z += fmaf(c.dt, c.gz, k * az);
-    vout[i] = vi;
+    vout[i].x = xi;
+    vout[i].v = vi;
 }
 
 // ---------------------------------------------------------------------------------------------
 // A11: implicit viscosity (Eq. 16-19; R4, R21, R23), matrix-free CG on
 // (I - dt A) v* = v~ with
 //   (A u)_i = 2(d+2) sum_j mu m / (rho_i rho_j) (u_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij.
-// Vectors are float4 with rho in .w.  out_i = u_i - dt (A u)_i when RESIDUAL0 = false;
+// Vectors are float4 with rho in .w (the start vector b = v~ lives in the PV records).  out_i = u_i - dt (A u)_i when RESIDUAL0 = false;
 // RESIDUAL0 = true is the start-up r0 = b - (I - dt A) b = dt A b (x0 = b = v~), which also seeds
 // the search direction and reduces |b|^2, |r0|^2.
 template <bool LIST, bool RESIDUAL0>
 __global__ void __launch_bounds__(kBlock)
-k_cg_apply(PassCtx p, const float4 *__restrict__ u, float4 *__restrict__ out,
+k_cg_apply(PassCtx p, const float4 *__restrict__ u /* RESIDUAL0: PV records */, float4 *__restrict__ out,
            float4 *__restrict__ out2, float *__restrict__ partial, float *__restrict__ partial2)
 {
     __shared__ float red[kBlock / 32];
@@ -725,9 +738,9 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u, float4 *__restrict__ out,
     float t1 = 0.f, t2 = 0.f;
     if (i < c.nf) {
         float4 xi = p.pos[i];
-        float4 ui = u[i];
+        float4 ui = RESIDUAL0 ? u[2 * i + 1] : u[i];
         float ax = 0.f, ay = 0.f, az = 0.f;
-        for_each_neighbor<LIST, false, 2>(p, p.pos, u, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, false, RESIDUAL0 ? 3 : 2>(p, RESIDUAL0 ? u : p.pos, u, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 uj, float dx, float dy, float dz, float d2) {
                 float du = fmaf(ui.x - uj.x, dx, fmaf(ui.y - uj.y, dy, (ui.z - uj.z) * dz));
                 float s = pair_gradf(c, d2) * du / ((d2 + c.visc_eps) * uj.w);
@@ -759,7 +772,7 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u, float4 *__restrict__ out,
 // x += a p;  r -= a Ap;  partial |r|^2
 __global__ void __launch_bounds__(256)
 k_cg_update(int n, const DevControl *__restrict__ ctl, const float4 *__restrict__ pd,
-            const float4 *__restrict__ Ap, float4 *__restrict__ x, float4 *__restrict__ r,
+            const float4 *__restrict__ Ap, PV *__restrict__ x, float4 *__restrict__ r,
             float *__restrict__ partial)
 {
     __shared__ float red[8];
@@ -767,10 +780,10 @@ k_cg_update(int n, const DevControl *__restrict__ ctl, const float4 *__restrict_
     float t = 0.f;
     if (i < n) {
         float a = (float)ctl->cg_alpha;
-        float4 pv = pd[i], av = Ap[i], xv = x[i], rv = r[i];
+        float4 pv = pd[i], av = Ap[i], xv = x[i].v, rv = r[i];
         xv.x = fmaf(a, pv.x, xv.x); xv.y = fmaf(a, pv.y, xv.y); xv.z = fmaf(a, pv.z, xv.z);
         rv.x = fmaf(-a, av.x, rv.x); rv.y = fmaf(-a, av.y, rv.y); rv.z = fmaf(-a, av.z, rv.z);
-        x[i] = xv; r[i] = rv;
+        x[i].v = xv; r[i] = rv;
         t = fmaf(rv.x, rv.x, fmaf(rv.y, rv.y, rv.z * rv.z));
     }
     float s = block_sum(t, red);
@@ -795,13 +808,13 @@ k_cg_direction(int n, const DevControl *__restrict__ ctl, const float4 *__restri
 // p = k((rho~/rho0)^gamma - 1), evaluated as k expm1(gamma log1p(delta)), delta = (rho~ - rho0)/rho0,
 // which keeps the small excess accurate in fp32.  posk.w = p / rho~^2 (vel.w keeps rho).
 __global__ void __launch_bounds__(256)
-k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const float4 *__restrict__ vel,
+k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const PV *__restrict__ pv,
             float4 *__restrict__ posk)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.nf) return;
     float4 x = pos[i];
-    float rho = vel[i].w;
+    float rho = pv[i].v.w;
     float rt = fmaxf(rho, c.rho0);
     float delta = (rt - c.rho0) / c.rho0;
     float pr = c.wc_k * expm1f(c.wc_gamma * log1pf(delta));

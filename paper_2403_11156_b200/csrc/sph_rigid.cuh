@@ -31,11 +31,12 @@ k_export_vec3(const float4 *__restrict__ src, const int *__restrict__ id, int n,
     out[3 * o] = v.x; out[3 * o + 1] = v.y; out[3 * o + 2] = v.z;
 }
 __global__ void __launch_bounds__(256)
-k_export_w(const float4 *__restrict__ src, const int *__restrict__ id, int n, float *__restrict__ out)
+k_export_w(const float4 *__restrict__ src, const int *__restrict__ id, int n, float *__restrict__ out,
+           int stride /* float4 elements between consecutive particles */)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
-    out[id != nullptr ? id[s] : s] = src[s].w;
+    out[id != nullptr ? id[s] : s] = src[(size_t)s * stride].w;
 }
 __global__ void __launch_bounds__(256)
 k_export_scalar(const float *__restrict__ src, const int *__restrict__ id, int n, float *__restrict__ out)
