@@ -95,23 +95,52 @@ def dist_env():
 # Algorithmic work per fluid particle of each kernel:
 # compulsory bytes = own inputs read once + outputs written once, neighbour gathers assumed
 # cache-served; nf / nbd = mean fluid / boundary neighbours, cand = mean candidates of the 27-cell walk.
+# Fluid list entries are 2 bytes, boundary entries 4 bytes.
 def kernel_work(name, nf_mean, nb_mean, cand_mean):
-    lst = 4.0 * (nf_mean + nb_mean)
-    if name == "k_density_alpha":      # A4 + list build: pos in; rho, alpha, count, list out
-        return dict(bytes=16 + 4 + 4 + 4 + lst, flops=8.0 * cand_mean + 34.0 * (nf_mean + nb_mean) + 25, row="A4")
-    if name == "k_solver_p":           # pos, vel, alpha, count, list in; posk out
-        return dict(bytes=16 + 16 + 4 + 4 + lst + 16, flops=27.0 * (nf_mean + nb_mean) + 12, row="A5/A7 P")
-    if name == "k_solver_c":           # posk, count, list, vel in; vel out
-        return dict(bytes=16 + 4 + lst + 16 + 16, flops=26.0 * (nf_mean + nb_mean) + 12, row="A5/A7 C")
-    if name == "k_reorder":            # slot, key, cell range, pos, vel, id in; pos, vel, id out
-        return dict(bytes=4 + 4 + 8 + 36 + 36, flops=0.0, row="A3")
+    lst = 2.0 * nf_mean + 4.0 * nb_mean
+    nn = nf_mean + nb_mean
+    if name == "k_build_lists":        # A4 walk: pos in; count, lists out; predicate R10 on every candidate
+        return dict(bytes=16 + 4 + lst, flops=8.0 * cand_mean, row="A4 (lists)")
+    if name == "k_density_alpha":      # record, count, list in; rho, alpha, posk out (+ fused first divergence P-pass)
+        return dict(bytes=32 + 4 + lst + 4 + 4 + 16, flops=45.0 * nn + 25, row="A4 + A5 P")
+    if name == "k_solver_p":           # record, alpha, count, list in; posk out
+        return dict(bytes=32 + 4 + 4 + lst + 16, flops=27.0 * nn + 12, row="A5/A7 P")
+    if name == "k_solver_c":           # posk, count, list, vel in; vel out; one launch in three also integrates (A9)
+        return dict(bytes=16 + 4 + lst + 16 + 16 + (4 + 36) / 3.0, flops=26.0 * nn + 12, row="A5/A7 C (+A6, A9)")
+    if name == "k_reorder":            # slot, key, cell range, pos, vel, id in; pos, record, id out
+        return dict(bytes=4 + 4 + 8 + 36 + 16 + 32 + 4, flops=0.0, row="A3")
     if name == "k_cell_key_hist":
         return dict(bytes=16 + 4 + 4 + 8, flops=10.0, row="A1")
-    if name == "k_integrate":
-        return dict(bytes=36 + 36, flops=12.0, row="A9")
-    if name == "k_gravity":
-        return dict(bytes=32, flops=6.0, row="A6")
     return None
+
+
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the config-4 launches in the
+# committed `ncu --set full` capture profiles/r1c_ncu_full_summary.md (another run of the same command
+# as the roofline's timing: context for `achieved`, not a live measurement)
+NCU_TRAFFIC_BYTES = {
+    ("config4_splash_1p23M", "k_solver_p"): 128.761088e6 + 11.352832e6,
+    ("config4_splash_1p23M", "k_solver_c"): 148.436736e6 + 45.320448e6,
+    ("config4_splash_1p23M", "k_build_lists"): 24.881152e6 + 25.545984e6,
+    ("config4_splash_1p23M", "k_density_alpha"): 143.713536e6 + 30.034432e6,
+}
+# l1tex__throughput.avg.pct_of_peak_sustained_active of the same capture: the list passes are bound by the
+# L1 gather path (see the profile), which is why their HBM fraction is low
+NCU_L1TEX_PCT = {"k_solver_p": 88.7, "k_solver_c": 78.8, "k_build_lists": 85.5, "k_density_alpha": 88.6}
+
+
+def max_over_ranks(ms_local, world, device):
+    """Replicas-only multi-GPU: the job's time is the slowest rank's."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(n_units_per_rank, steps, ms_max, world):
+    """Whole-job particle-steps/s: every rank advanced its own replica by `steps` steps in ms_max."""
+    return world * n_units_per_rank * steps / (ms_max * 1e-3)
 
 
 def run_ours(args):
@@ -155,12 +184,9 @@ def run_ours(args):
     ms = e0.elapsed_time(e1)
     st1 = sim.sph_read_stats()
     launches = sim.sph_launch_count() - launches0
-    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms_max = float(tms.item())
+    ms_max = max_over_ranks(ms, world, "cuda")
     nf = sc.n_fluid
-    value = world * nf * K / (ms_max * 1e-3)
+    value = job_throughput(nf, K, ms_max, world)
     mean_it_v = (st1["total_it_v"] - st0["total_it_v"]) / max(K, 1)
     mean_it_d = (st1["total_it_d"] - st0["total_it_d"]) / max(K, 1)
 
@@ -186,10 +212,7 @@ def run_ours(args):
     wall = time.perf_counter() - t0
     barrier()
     ems = max(e0.elapsed_time(e1), wall * 1e3)
-    tms = torch.tensor([ems], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    e2e_value = world * nf * Ke / (float(tms.item()) * 1e-3)
+    e2e_value = job_throughput(nf, Ke, max_over_ranks(ems, world, "cuda"), world)
     sim.close()
 
     out = None
@@ -238,12 +261,15 @@ def run_ours(args):
         dur = 1e-3 * kt[top][1] / kt[top][0]
         fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roof = {"kernel": top, "row": work["row"] if work else None, "avg_us": round(dur * 1e6, 2),
-                "share_of_step": table[top]["share"], "traffic": None,
+                "share_of_step": table[top]["share"], "traffic": NCU_TRAFFIC_BYTES.get((sc.name, top)),
+                "traffic_source": "profiles/r1c_ncu_full_summary.md" if (sc.name, top) in NCU_TRAFFIC_BYTES else None,
+                "l1tex_throughput_pct_ncu": NCU_L1TEX_PCT.get(top),
                 "peak_source": peaks["source"] + " (MEASURED_PEAKS.json)"}
         if work:
             gbs = work["bytes"] * nf / dur / 1e9
             tfl = work["flops"] * nf / dur / 1e12
-            if top == "k_density_alpha":
+            roof["algorithmic_bytes"] = work["bytes"] * nf
+            if top == "k_build_lists":
                 roof.update({"bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s",
                              "frac": tfl / fp32_peak, "hbm_achieved_gbs": gbs, "hbm_frac": gbs / peaks["hbm_gbs"]})
             else:
