@@ -157,7 +157,11 @@ def run_ours(args):
     B.load()
     peaks = load_peaks()
 
-    sc = scenes.config(args.config, seed=rank)
+    if args.n_target:
+        # scaling sweep of BASELINE.json configs[4]: the config-4 scene with every site count scaled
+        sc = scenes.splash(n_target=args.n_target, seed=rank, name="config4_splash_sweep_%.3gM" % (args.n_target / 1e6))
+    else:
+        sc = scenes.config(args.config, seed=rank)
     K, W = args.steps, args.warmup
     sim = B.Sim.from_scene(sc, device=local_rank, use_cuda_graph=0 if args.no_graph else 1)
     stream = sim.stream
@@ -378,6 +382,9 @@ def main():
     ap.add_argument("--no-graph", action="store_true",
                     help="host-driven launches instead of the CUDA graph (ncu cannot profile kernel nodes of a "
                          "graph that has conditional nodes): for profiling commands only")
+    ap.add_argument("--n-target", type=float, default=0.0,
+                    help="scaling sweep: config-4 scene proportions at this many fluid particles (250e3 / 4e6 / 8e6); "
+                         "not the headline line")
     ap.add_argument("--no-breakdown", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

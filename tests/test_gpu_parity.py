@@ -373,6 +373,34 @@ def test_config4_full_size_sampled_parity(B, oracle):
     g.close()
 
 
+@pytest.mark.parametrize("idx,warm", [(1, 4), (2, 4), (3, 2), (4, 6)])
+def test_full_size_whole_step_parity(B, oracle, idx, warm):
+    """BASELINE configs 1-4 at FULL size in the configuration bench.py times (CUDA graph, neighbour
+    lists): a few free-running GPU steps, then one resynchronised step on both sides (oracle forced to
+    the GPU's iteration counts, R20): rho, alpha, v within 1e-4, x within dt * 1e-4 * vscale; the
+    density solve leaves err_rho < 0.1 %.  Config 1 also takes one resynchronised WCSPH step."""
+    import torch
+    sc = scenes.config(idx)
+    g, o = make_pair(sc, oracle)
+    if idx == 3:
+        # the free-falling column has a uniform velocity (A v = 0, CG exits at once): shear it
+        x = g.sph_read_state(B.POS)
+        v0 = torch.zeros_like(x)
+        v0[:, 0] = 2.0 * torch.sin(25.0 * x[:, 2]); v0[:, 1] = 1.5 * torch.cos(30.0 * x[:, 0]); v0[:, 2] = -1.0
+        g.sph_write_state(B.VEL, v0)
+    g.sph_step_dfsph(warm)
+    e, st = resync_step(g, o, sc)
+    check_errors(e, sc)
+    assert st["overflow_count"] == 0 and st["nan_count"] == 0 and st["oob_count"] == 0, st
+    assert st["err_rho"] < 1e-3 and st["it_d"] >= 2, st
+    if idx == 3:
+        assert st["cg_iters"] == o.stats()["cg_iters"] > 0
+    if idx == 1:
+        e, st = resync_step(g, o, sc, method="wcsph")
+        check_errors(e, sc)
+    g.close(); o.close()
+
+
 def torch_index(a):
     import torch
     return torch.as_tensor(np.asarray(a), dtype=torch.long, device="cuda")
