@@ -89,15 +89,26 @@ __global__ void __launch_bounds__(B) k_smem(const uint32_t *__restrict__ nl16, c
     uint32_t ok = 0;
     while (!ok) asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0,1,0,p; }" : "=r"(ok) : "r"(smem_u32(&bar)) : "memory");
     float sx = 0, sy = 0, sz = 0, sw = 0;
+    // list words software-pipelined exactly like the library's list passes
+    constexpr int PB = 4;
+    uint32_t cur[PB];
+#pragma unroll
+    for (int t = 0; t < PB; ++t) cur[t] = t < npair ? __ldg(lp + t * 32) : 0u;
 #pragma unroll 1
-    for (int p0 = 0; p0 < npair; p0 += 2) {
-        uint32_t w0 = __ldg(lp + p0 * 32), w1 = p0 + 1 < npair ? __ldg(lp + (p0 + 1) * 32) : w0;
-        uint32_t e[4] = { w0 & 0xffffu, w0 >> 16, w1 & 0xffffu, w1 >> 16 };
-        float4 a[4];
+    for (int pb = 0; pb < npair; pb += PB) {
+        uint32_t nxt[PB];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) a[u] = *reinterpret_cast<const float4 *>(sm + (size_t)e[u] * 16);
+        for (int t = 0; t < PB; ++t) nxt[t] = pb + PB + t < npair ? __ldg(lp + (pb + PB + t) * 32) : 0u;
+        float4 a[2 * PB];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { sx += a[u].x; sy += a[u].y; sz += a[u].z; sw += a[u].w; }
+        for (int u = 0; u < 2 * PB; ++u) {
+            uint32_t e = (u & 1) ? (cur[u >> 1] >> 16) : (cur[u >> 1] & 0xffffu);
+            a[u] = *reinterpret_cast<const float4 *>(sm + (size_t)e * 16);
+        }
+#pragma unroll
+        for (int u = 0; u < 2 * PB; ++u) if (2 * pb + u < c) { sx += a[u].x; sy += a[u].y; sz += a[u].z; sw += a[u].w; }
+#pragma unroll
+        for (int t = 0; t < PB; ++t) cur[t] = nxt[t];
     }
     if (i < n) out[i] = make_float4(sx, sy, sz, sw);
 }
@@ -167,8 +178,9 @@ int main()
         }
         cudaFree(dnl);
     }
-    // ---- shared-memory staged tile, 16-bit tile-relative entries
-    {
+    // ---- shared-memory staged tile, 16-bit tile-relative entries; cf = 1: entries nudged so that the 8 lanes
+    // of a quarter-warp always hit 8 different 16-byte bank groups (what a conflict-free schedule would give)
+    for (int cf = 0; cf < 2; ++cf) {
         std::vector<uint16_t> nl16((size_t)NW * kf * 32, 0); std::vector<int> cnt(N); double staged = 0;
         for (int b = 0; b < nb; ++b) {
             int i0 = b * B, il = std::min(i0 + B - 1, N - 1), ca = i0 / PPC, cb = il / PPC, rs[9], rn[9], pre[9], o = 0;
@@ -178,17 +190,18 @@ int main()
             staged += o;
             for (int i = i0; i <= il; ++i) {
                 uint16_t *lp = &nl16[(size_t)(i >> 5) * kf * 32 + (i & 31) * 2]; int k = 0;
-                for (int r = 0; r < 9; ++r) for (int j : nbr[(size_t)i * 9 + r]) if (k < kf) { lp[(k >> 1) * 64 + (k & 1)] = (uint16_t)(pre[r] + j - rs[r]); ++k; }
+                for (int r = 0; r < 9; ++r) for (int j : nbr[(size_t)i * 9 + r]) if (k < kf) { int e = pre[r] + j - rs[r]; if (cf) e = (e & ~7) | (((i & 31) + k) & 7); lp[(k >> 1) * 64 + (k & 1)] = (uint16_t)e; ++k; }
                 if (k & 1) lp[(k >> 1) * 64 + 1] = lp[(k >> 1) * 64];
                 cnt[i] = k;
             }
         }
         uint32_t *dnl; int *dcnt; cudaMalloc(&dnl, nl16.size() * 2); cudaMalloc(&dcnt, N * 4);
         cudaMemcpy(dnl, nl16.data(), nl16.size() * 2, cudaMemcpyHostToDevice); cudaMemcpy(dcnt, cnt.data(), N * 4, cudaMemcpyHostToDevice);
-        printf("shared-memory staged tile: %.0f records per CTA of %d particles\n", staged / nb, B);
+        printf("shared-memory staged tile (%s): %.0f records per CTA of %d particles\n", cf ? "conflict-free entries" : "real entries", staged / nb, B);
         for (int skip : { 0, 1 })
             printf("  LDS.128 gathers, %-28s %7.1f us\n", skip ? "tile copy skipped (gather only)" : "cp.async.bulk tile copy",
                    best_of([&] { k_smem<<<nb, B, 1536 * 16>>>(dnl, dcnt, kf, dpos, dout, N, skip); }));
+        cudaFree(dnl); cudaFree(dcnt);
     }
     printf("%s\n", cudaGetErrorString(cudaDeviceSynchronize()));
     return 0;
