@@ -404,3 +404,64 @@ def test_full_size_whole_step_parity(B, oracle, idx, warm):
 def torch_index(a):
     import torch
     return torch.as_tensor(np.asarray(a), dtype=torch.long, device="cuda")
+
+
+# ------------------------------------------------------------------ full length, all five configs
+
+def _run_full(B, sc, n_steps, method="dfsph", chunk=1):
+    """Free-running GPU simulation of a BASELINE config for its full length; statistics are read
+    after every `chunk` steps.  Returns (sim, list of stats)."""
+    g = B.Sim.from_scene(sc)
+    hist = []
+    done = 0
+    while done < n_steps:
+        k = min(chunk, n_steps - done)
+        (g.sph_step_dfsph if method == "dfsph" else g.sph_step_wcsph)(k)
+        done += k
+        hist.append(g.sph_read_stats())
+    return g, hist
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_full_length_run_converges_on_every_step(B, idx):
+    """north_star: "DFSPH converging to average density error < 0.1 %" -- every step of every
+    BASELINE config at full size and full length (100 / 500 / 1000 / 500 / 200 steps), in the
+    configuration bench.py times.  Also: no NaN, no list overflow, nothing outside the grid, the
+    iteration limits never hit, all particles still inside the tank at the end."""
+    sc = scenes.config(idx)
+    n_steps = int(sc.steps)
+    g, hist = _run_full(B, sc, n_steps)
+    assert hist[-1]["steps_done"] == n_steps
+    worst = max(h["err_rho"] for h in hist)
+    assert worst < 1e-3, worst
+    for h in hist:
+        assert h["nan_count"] == 0 and h["overflow_count"] == 0 and h["oob_count"] == 0, h
+        assert h["max_iter_hit"] == 0, h
+        assert h["it_d"] >= 2 and h["it_v"] >= 1, h
+        if idx == 3:
+            assert h["cg_residual"] <= 1.5e-5, h
+    p = np_(g.sph_read_state(B.POS))
+    lo, hi = np.asarray(sc.params["tank_min"]), np.asarray(sc.params["tank_max"])
+    h_ = sc.params["support_radius"]
+    assert np.isfinite(p).all() and (p > lo - h_).all() and (p < hi + h_).all()
+    rho = np_(g.sph_read_state(B.DENSITY))
+    assert rho.max() < 1.05 * sc.params["rest_density"], rho.max()
+    g.close()
+
+
+def test_config1_wcsph_and_dfsph_centre_of_mass_agree(B):
+    """BASELINE config 1 cross-check at full size: the same dam break run with DFSPH (dt = 4e-4)
+    and WCSPH (k = 5e4, gamma = 7, dt = 1e-4) to the same physical time 0.06 s; fluid centres of mass
+    within 0.25 particle diameters (the oracle's own cross-check pin, here on the GPU path)."""
+    sc = scenes.config(1)
+    g, _ = _run_full(B, sc, 150, chunk=150)
+    com_d = np_(g.sph_read_state(B.POS)).astype(np.float64).mean(axis=0)
+    g.close()
+    scw = scenes.dam_break((50, 50, 50), (100, 50, 50), r=0.01, dt=1e-4, steps=2000, name="config1_wcsph",
+                           viscosity_mode=1, kinematic_viscosity=0.01)
+    g, hist = _run_full(B, scw, 600, method="wcsph", chunk=600)
+    assert hist[-1]["nan_count"] == 0
+    com_w = np_(g.sph_read_state(B.POS)).astype(np.float64).mean(axis=0)
+    g.close()
+    d = 2.0 * sc.params["particle_radius"]
+    assert np.linalg.norm(com_d - com_w) <= 0.25 * d, (com_d, com_w)
