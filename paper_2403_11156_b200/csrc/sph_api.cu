@@ -174,6 +174,7 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     double sigma = 8.0 / (3.14159265358979323846 * hd * hd * hd);   // R1
     c.sigma = (float)sigma;
     c.grad_c = (float)(sigma / hd);
+    c.ga = (float)(18.0 / (hd * hd)); c.gb = (float)(-12.0 / hd); c.half_h = 0.5f * c.h;
     double d = 2.0 * (double)p.particle_radius;
     c.m = p.particle_mass > 0.f ? p.particle_mass : (float)((double)p.rest_density * d * d * d);   // R3
     c.rho0 = p.rest_density; c.dt = p.dt;

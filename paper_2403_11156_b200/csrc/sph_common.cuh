@@ -29,6 +29,8 @@ struct SimConst {
     float h, h2, inv_h;  // support radius, h*h in fp32 (R10), 1/h
     float sigma;         // 8 / (pi h^3)           (R1)
     float grad_c;        // sigma / h
+    float ga, gb;        // gradient factor of the inner branch: 6 (3q - 2) / h = ga r + gb, ga = 18 / h^2, gb = -12 / h
+    float half_h;        // branch point q = 1/2 in terms of r
     float m;             // fluid particle mass     (R3)
     float rho0, dt;
     float gx, gy, gz;
@@ -119,10 +121,13 @@ __device__ __forceinline__ float spline_gradf(float q, float rinv, float inv_h)
     return q <= 0.5f ? a : b;
 }
 
-// r and 1/r from d2 (d2 > 0 for the second branch; guarded for d2 == 0).
+// r and 1/r from d2 (d2 > 0 for the second branch; guarded for d2 == 0).  The argument of the
+// reciprocal square root is never denormal (>= 1e-30), so the flush-to-zero MUFU form returns the
+// same value as rsqrtf() without its denormal pre-/post-scaling instructions.
 __device__ __forceinline__ void r_and_rinv(float d2, float &r, float &rinv)
 {
-    rinv = rsqrtf(fmaxf(d2, 1e-30f));
+    float a = fmaxf(d2, 1e-30f);
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(a));
     r = d2 * rinv;
 }
 

@@ -206,9 +206,14 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
 // gradient factor for a pair at squared distance d2: grad_i W_ij = grad_c * gf * d
 __device__ __forceinline__ float pair_gradf(const SimConst &c, float d2)
 {
+    // spline_gradf(r / h, 1 / r, 1 / h) with the constants folded (R1): inner branch 6 (3q - 2) / h = ga r + gb,
+    // outer branch -6 (1 - q)^2 / r
     float r, rinv;
     r_and_rinv(d2, r, rinv);
-    return spline_gradf(r * c.inv_h, rinv, c.inv_h);
+    float a = fmaf(r, c.ga, c.gb);
+    float t = fmaf(r, -c.inv_h, 1.0f);
+    float b = (t * t) * (-6.0f * rinv);
+    return r <= c.half_h ? a : b;
 }
 
 // ---------------------------------------------------------------------------------------------
