@@ -26,6 +26,13 @@ enum { MODE_DIV = 0, MODE_DENS = 1 };
 struct __align__(32) PV { float4 x, v; };   // position (x, y, z, -) | velocity (vx, vy, vz, rho)
 
 // 32 bytes (aligned) through the read-only path with one instruction
+__device__ __forceinline__ void ldg256_if(bool on, const float4 *p, float4 &a, float4 &b)
+{
+    asm("{\n\t.reg .pred pp;\n\tsetp.ne.u32 pp, %9, 0;\n\t"
+        "@pp ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n\t}"
+        : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
+        : "l"(p), "r"((unsigned)on));
+}
 __device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b)
 {
     asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -157,9 +164,12 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
                 e = valid ? e : 0u;                       // the unwritten half of an odd tail pair is garbage
                 int j = tbl[(e >> kOffBits) * kBlock] + (int)(e & kOffMask);
                 jj[u] = valid ? j : i;
-                if (NSRC == 3) ldg256(src + 2 * jj[u], q[u], q2[u]);
+                // predicated record gather: a lane whose list has ended issues no memory access at all (its registers
+                // stay undefined and are never read -- the arithmetic below is under the same predicate); the record
+                // passes are bound by L1 wavefronts, and ended lanes would each touch their own record's line
+                if (NSRC == 3) ldg256_if(valid, src + 2 * jj[u], q[u], q2[u]);
                 else {
-                    q[u] = __ldg(src + jj[u]);
+                    q[u] = __ldg(src + jj[u]);       // (measured: predication costs the issue-bound C-pass more than it saves)
                     if (NSRC == 2) q2[u] = __ldg(src2 + jj[u]);
                 }
             }
