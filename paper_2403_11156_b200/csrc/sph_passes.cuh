@@ -133,7 +133,11 @@ __device__ __forceinline__ void fill_run_table(const Geom &g, const int *__restr
 // LIST = false: walk the cells and evaluate the predicate (same visiting order, same arithmetic).
 // `src` is the float4 array whose xyz are the neighbour positions (pos or posk);
 // WITH_B = false skips the boundary part.  tbl: kRows * kBlock ints of shared memory (LIST only).
-template <bool LIST, bool WITH_B, int NSRC, class FF, class FB>
+// PADSAFE (NSRC 1 or 2, LIST): ff is also called for the slots past the end of a lane's list, with the
+//   lane's OWN record as the neighbour (d = 0 exactly): legal when every term ff accumulates carries a
+//   factor d (or v_i - v_j), so that such a call adds exactly 0 -- it removes one branch per slot from
+//   the issue-bound C-pass.
+template <bool LIST, bool WITH_B, int NSRC, bool PADSAFE, class FF, class FB>
 __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4 *__restrict__ src,
                                                   const float4 *__restrict__ src2, int *tbl_base,
                                                   int i, float xi, float yi, float zi, FF &&ff, FB &&fb)
@@ -175,7 +179,7 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
             }
 #pragma unroll
             for (int u = 0; u < 2 * PB; ++u) {
-                if (2 * pb + u < cf) {
+                if ((PADSAFE && NSRC != 3) || 2 * pb + u < cf) {
                     float dx = __fsub_rn(xi, q[u].x), dy = __fsub_rn(yi, q[u].y), dz = __fsub_rn(zi, q[u].z);
                     ff(jj[u], q[u], NSRC >= 2 ? q2[u] : q[u], dx, dy, dz, dist2_r10(dx, dy, dz));
                 }
@@ -512,7 +516,7 @@ k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
         float sw = 0.f, sx = 0.f, sy = 0.f, sz = 0.f, t2 = 0.f;    // fluid: sum w, sum gf d, sum gf^2 d2
         float bw = 0.f, bx = 0.f, by = 0.f, bz = 0.f;              // boundary, Psi-weighted
         float df = 0.f, db = 0.f;                                  // density rate (DIVP)
-        for_each_neighbor<LIST, true, DIVP ? 3 : 1>(p, DIVP ? reinterpret_cast<const float4 *>(pv) : p.pos, nullptr, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, true, DIVP ? 3 : 1, false>(p, DIVP ? reinterpret_cast<const float4 *>(pv) : p.pos, nullptr, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
                 float r, rinv;
                 r_and_rinv(d2, r, rinv);
@@ -584,7 +588,7 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
         float4 xi, vi;
         ldg256(reinterpret_cast<const float4 *>(pv + i), xi, vi);
         float df = 0.f, db = 0.f;
-        for_each_neighbor<LIST, true, 3>(p, reinterpret_cast<const float4 *>(pv), nullptr, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, true, 3, false>(p, reinterpret_cast<const float4 *>(pv), nullptr, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
                 float gf = pair_gradf(c, d2);
                 float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
@@ -651,7 +655,7 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, PV *__restrict__ pv, CTai
         float4 xi = posk[i];
         float kri = xi.w;
         float fx = 0.f, fy = 0.f, fz = 0.f, bx = 0.f, by = 0.f, bz = 0.f;
-        for_each_neighbor<LIST, true, 1>(p, posk, posk, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, true, 1, true>(p, posk, posk, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4 pj, float4, float dx, float dy, float dz, float d2) {
                 float s = (kri + pj.w) * pair_gradf(c, d2);
                 fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz);
@@ -718,7 +722,7 @@ k_explicit_viscosity(PassCtx p, const PV *__restrict__ vin, PV *__restrict__ vou
     float4 xi, vi;
     ldg256(reinterpret_cast<const float4 *>(vin + i), xi, vi);
     float ax = 0.f, ay = 0.f, az = 0.f;
-    for_each_neighbor<LIST, false, 3>(p, reinterpret_cast<const float4 *>(vin), nullptr, tbl, i, xi.x, xi.y, xi.z,
+    for_each_neighbor<LIST, false, 3, false>(p, reinterpret_cast<const float4 *>(vin), nullptr, tbl, i, xi.x, xi.y, xi.z,
         [&](int, float4, float4 vj, float dx, float dy, float dz, float d2) {
             float dv = fmaf(vi.x - vj.x, dx, fmaf(vi.y - vj.y, dy, (vi.z - vj.z) * dz));
             float rj = CLAMP ? fmaxf(vj.w, c.rho0) : vj.w;
@@ -755,7 +759,7 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u /* RESIDUAL0: PV records */, 
         float4 xi = p.pos[i];
         float4 ui = RESIDUAL0 ? u[2 * i + 1] : u[i];
         float ax = 0.f, ay = 0.f, az = 0.f;
-        for_each_neighbor<LIST, false, RESIDUAL0 ? 3 : 2>(p, RESIDUAL0 ? u : p.pos, u, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, false, RESIDUAL0 ? 3 : 2, !RESIDUAL0>(p, RESIDUAL0 ? u : p.pos, u, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 uj, float dx, float dy, float dz, float d2) {
                 float du = fmaf(ui.x - uj.x, dx, fmaf(ui.y - uj.y, dy, (ui.z - uj.z) * dz));
                 float s = pair_gradf(c, d2) * du / ((d2 + c.visc_eps) * uj.w);
