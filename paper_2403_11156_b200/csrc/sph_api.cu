@@ -151,7 +151,10 @@ bool make_geom(const SphParams &p, Geom &g, std::string &why)
     }
     long long nc = n[0] * n[1] * n[2];
     if (nc > 2000000000LL) { why = "grid exceeds 2^31 cells"; return false; }
-    g.nx = (int)n[0]; g.ny = (int)n[1]; g.nz = (int)n[2]; g.ncells = (int)nc;
+    if (nc * kFineX > 2000000000LL) { why = "grid exceeds 2^31 cells"; return false; }
+    g.nxc = (int)n[0]; g.ncells_c = (int)nc;
+    g.nx = (int)n[0] * kFineX; g.ny = (int)n[1]; g.nz = (int)n[2]; g.ncells = (int)nc * kFineX;
+    g.inv_cx = g.inv_c * (float)kFineX;
     return true;
 }
 
@@ -550,7 +553,7 @@ struct FieldInfo { size_t bytes; bool writable; bool derived; };
 
 bool field_info(const SphSim *s, int field, FieldInfo &fi)
 {
-    const size_t nf = (size_t)s->c.nf, nb = (size_t)s->c.nb, nc1 = (size_t)s->c.g.ncells + 1;
+    const size_t nf = (size_t)s->c.nf, nb = (size_t)s->c.nb, nc1 = (size_t)s->c.g.ncells_c + 1;
     switch (field) {
     case SPH_FIELD_POS: case SPH_FIELD_VEL: fi = { nf * 12, true, false }; return true;
     case SPH_FIELD_DENSITY: case SPH_FIELD_ALPHA: case SPH_FIELD_KAPPA_OVER_RHO: fi = { nf * 4, false, true }; return true;
@@ -582,9 +585,9 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
     case SPH_FIELD_ALPHA: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->alpha, s->idB, nf, (float *)out); break;
     case SPH_FIELD_KAPPA_OVER_RHO: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posk, s->idB, nf, (float *)out, 1); break;
     case SPH_FIELD_CELL_START:
-        CUDA_TRY(s, cudaMemcpyAsync(out, s->gf.cell_start, bytes, cudaMemcpyDeviceToDevice, st)); break;
+        LAUNCH(s, k_export_cell_start, cdiv(s->c.g.ncells_c + 1, 256), 256, st, s->gf.cell_start, s->c.g.ncells_c + 1, (int *)out); break;
     case SPH_FIELD_BOUNDARY_CELL_START:
-        CUDA_TRY(s, cudaMemcpyAsync(out, s->gb.cell_start, bytes, cudaMemcpyDeviceToDevice, st)); break;
+        LAUNCH(s, k_export_cell_start, cdiv(s->c.g.ncells_c + 1, 256), 256, st, s->gb.cell_start, s->c.g.ncells_c + 1, (int *)out); break;
     case SPH_FIELD_CELL_OF_PARTICLE:
         LAUNCH(s, k_export_keys, cdiv(nf, 256), 256, st, s->posB, s->idB, nf, s->c.g, (int *)out); break;
     case SPH_FIELD_BOUNDARY_CELL_OF_PARTICLE:
@@ -646,7 +649,7 @@ int sph_grid_dims(const SphParams *params, int dims[4], int caps[2])
     Geom g;
     std::string why;
     if (!make_geom(*params, g, why)) return SPH_EDOMAIN;
-    if (dims) { dims[0] = g.nx; dims[1] = g.ny; dims[2] = g.nz; dims[3] = g.ncells; }
+    if (dims) { dims[0] = g.nxc; dims[1] = g.ny; dims[2] = g.nz; dims[3] = g.ncells_c; }
     if (caps) { caps[0] = list_cap(params->max_fluid_neighbors, kMaxListCap); caps[1] = list_cap(params->max_boundary_neighbors, 65532); }
     return SPH_OK;
 }

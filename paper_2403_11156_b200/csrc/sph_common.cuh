@@ -16,9 +16,18 @@ constexpr int kBigCell = 2048;     // cells above this size keep atomic order (R
 
 // Uniform grid geometry (reading R11): cell edge c = h (1 + 2^-10) in fp32, origin = domain_min,
 // n_a = floor((max_a - o_a) * inv_c) + 1, linear key x-fastest.
+// Internally every R11 cell is split into kFineX slabs along x ("fine cells"): the store is sorted by
+// fine key, and the x-run of a particle in fine cell f is the fine cells [f - kFineX, f + kFineX] =
+// (2 + 1/kFineX) c wide instead of 3 c -- fewer candidates for the list builder.  Multiplying the
+// fp32 cell coordinate t = (x - o) * inv_c by a power of two is exact, so floor(kFineX t) / kFineX =
+// floor(t): the R11 cell of a particle is its fine cell / kFineX, and because the key is x-fastest
+// the R11 cell_start is every kFineX-th entry of the fine one (what the ABI exports).
+constexpr int kFineX = 2;          // power of two
 struct Geom {
     float ox, oy, oz, inv_c;
-    int nx, ny, nz, ncells;
+    float inv_cx;                  // kFineX * inv_c
+    int nx, ny, nz, ncells;        // FINE cell counts (nx = kFineX * R11 nx)
+    int nxc, ncells_c;             // R11 (coarse) counts
 };
 
 // Per-simulation constants handed to kernels by value.
@@ -81,11 +90,12 @@ __device__ __forceinline__ int cell_coord(float x, float o, float inv_c, int n, 
     return (int)floorf(t);
 }
 
+// FINE key and coordinates (cx is the fine x coordinate)
 __device__ __forceinline__ int cell_key(const Geom &g, float x, float y, float z, bool &clamped,
                                         int &cx, int &cy, int &cz)
 {
     clamped = false;
-    cx = cell_coord(x, g.ox, g.inv_c, g.nx, clamped);
+    cx = cell_coord(x, g.ox, g.inv_cx, g.nx, clamped);
     cy = cell_coord(y, g.oy, g.inv_c, g.ny, clamped);
     cz = cell_coord(z, g.oz, g.inv_c, g.nz, clamped);
     return cx + g.nx * (cy + g.ny * cz);

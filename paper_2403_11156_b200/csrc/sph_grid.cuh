@@ -36,7 +36,8 @@ k_export_keys(const float4 *__restrict__ pos, const int *__restrict__ id, int n,
     if (s >= n) return;
     float4 p = pos[s];
     bool clamped; int cx, cy, cz;
-    out[id[s]] = cell_key(g, p.x, p.y, p.z, clamped, cx, cy, cz);
+    cell_key(g, p.x, p.y, p.z, clamped, cx, cy, cz);
+    out[id[s]] = cx / kFineX + g.nxc * (cy + g.ny * cz);           // the R11 key
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -195,6 +196,14 @@ k_reorder(const int *__restrict__ slot_src, const int *__restrict__ key,
         b_out[2 * dst + 1] = b_in[src];
     } else if (b_in != nullptr) b_out[dst] = b_in[src];
     id_out[dst] = id_in != nullptr ? id_in[src] : src;
+}
+
+// R11 cell_start = every kFineX-th entry of the fine one (n = coarse cells + 1 entries)
+__global__ void __launch_bounds__(256)
+k_export_cell_start(const int *__restrict__ fine, int n, int *__restrict__ out)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = fine[(size_t)k * kFineX];
 }
 
 }  // namespace sph

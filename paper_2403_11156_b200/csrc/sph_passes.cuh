@@ -68,7 +68,7 @@ __device__ __forceinline__ CellOf cell_of(const Geom &g, float x, float y, float
 {
     CellOf c; bool cl;
     cell_key(g, x, y, z, cl, c.cx, c.cy, c.cz);
-    c.x0 = max(c.cx - 1, 0); c.x1 = min(c.cx + 1, g.nx - 1);
+    c.x0 = max(c.cx - kFineX, 0); c.x1 = min(c.cx + kFineX, g.nx - 1);
     return c;
 }
 
