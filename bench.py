@@ -115,17 +115,19 @@ def kernel_work(name, nf_mean, nb_mean, cand_mean):
 
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the config-4 launches in the
-# committed `ncu --set full` capture profiles/r1c_ncu_full_summary.md (another run of the same command
+# committed `ncu --set full` capture profiles/r1d_ncu_full_summary.md (another run of the same command
 # as the roofline's timing: context for `achieved`, not a live measurement)
+NCU_PROFILE = "profiles/r1d_ncu_full_summary.md"
 NCU_TRAFFIC_BYTES = {
-    ("config4_splash_1p23M", "k_solver_p"): 128.761088e6 + 11.352832e6,
-    ("config4_splash_1p23M", "k_solver_c"): 148.436736e6 + 45.320448e6,
-    ("config4_splash_1p23M", "k_build_lists"): 24.881152e6 + 25.545984e6,
-    ("config4_splash_1p23M", "k_density_alpha"): 143.713536e6 + 30.034432e6,
+    ("config4_splash_1p23M", "k_solver_p"): 129.498624e6 + 12.624128e6,
+    ("config4_splash_1p23M", "k_solver_c"): 149.176576e6 + 44.282368e6,
+    ("config4_splash_1p23M", "k_build_lists"): 26.509056e6 + 27.070976e6,
+    ("config4_splash_1p23M", "k_density_alpha"): 144.399616e6 + 31.389440e6,
 }
 # l1tex__throughput.avg.pct_of_peak_sustained_active of the same capture: the list passes are bound by the
 # L1 gather path (see the profile), which is why their HBM fraction is low
-NCU_L1TEX_PCT = {"k_solver_p": 88.7, "k_solver_c": 78.8, "k_build_lists": 85.5, "k_density_alpha": 88.6}
+NCU_L1TEX_PCT = {"k_solver_p": 88.8, "k_solver_c": 86.8, "k_build_lists": 80.8, "k_density_alpha": 86.8}
+FINE_X = 2      # the library splits every grid cell into 2 slabs along x: x-runs cover 2.5 of the 3 cell widths
 
 
 def max_over_ranks(ms_local, world, device):
@@ -252,7 +254,7 @@ def run_ours(args):
         occ = (cs[1:] - cs[:-1]).to(torch.float32).reshape(1, 1, sim2.nz, sim2.ny, sim2.nx)
         # candidates per particle of the 27-cell walk = occupancy of the 3x3x3 cell box around it
         box = 27.0 * torch.nn.functional.avg_pool3d(occ, 3, stride=1, padding=1, count_include_pad=True)
-        cand_mean = float((occ * box).sum() / max(float(occ.sum()), 1.0))
+        cand_mean = float((occ * box).sum() / max(float(occ.sum()), 1.0)) * (2.0 + 1.0 / FINE_X) / 3.0
         sim2.sph_enable_kernel_timing(True)
         sim2.sph_step_dfsph(K)
         kt = sim2.sph_read_kernel_times()
@@ -266,7 +268,7 @@ def run_ours(args):
         fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
         roof = {"kernel": top, "row": work["row"] if work else None, "avg_us": round(dur * 1e6, 2),
                 "share_of_step": table[top]["share"], "traffic": NCU_TRAFFIC_BYTES.get((sc.name, top)),
-                "traffic_source": "profiles/r1c_ncu_full_summary.md" if (sc.name, top) in NCU_TRAFFIC_BYTES else None,
+                "traffic_source": NCU_PROFILE if (sc.name, top) in NCU_TRAFFIC_BYTES else None,
                 "l1tex_throughput_pct_ncu": NCU_L1TEX_PCT.get(top),
                 "peak_source": peaks["source"] + " (MEASURED_PEAKS.json)"}
         if work:
