@@ -26,6 +26,13 @@ enum { MODE_DIV = 0, MODE_DENS = 1 };
 struct __align__(32) PV { float4 x, v; };   // position (x, y, z, -) | velocity (vx, vy, vz, rho)
 
 // 32 bytes (aligned) through the read-only path with one instruction
+// list words are read once per pass: keep them out of L1, which the gathers need
+__device__ __forceinline__ uint32_t ldg_stream(const uint32_t *p)
+{
+    uint32_t v;
+    asm("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void ldg256_if(bool on, const float4 *p, float4 &a, float4 &b)
 {
     asm("{\n\t.reg .pred pp;\n\tsetp.ne.u32 pp, %9, 0;\n\t"
@@ -153,12 +160,12 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
         const int npair = (cf + 1) >> 1;
         uint32_t cur[PB];
 #pragma unroll
-        for (int t = 0; t < PB; ++t) cur[t] = t < npair ? __ldg(lp + t * 32) : 0u;
+        for (int t = 0; t < PB; ++t) cur[t] = t < npair ? ldg_stream(lp + t * 32) : 0u;
 #pragma unroll 1
         for (int pb = 0; pb < npair; pb += PB) {
             uint32_t nxt[PB];
 #pragma unroll
-            for (int t = 0; t < PB; ++t) nxt[t] = pb + PB + t < npair ? __ldg(lp + (pb + PB + t) * 32) : 0u;
+            for (int t = 0; t < PB; ++t) nxt[t] = pb + PB + t < npair ? ldg_stream(lp + (pb + PB + t) * 32) : 0u;
             int jj[2 * PB];
             float4 q[2 * PB], q2[NSRC >= 2 ? 2 * PB : 1];
 #pragma unroll
