@@ -711,6 +711,7 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
             CARVE((k_cg_apply<true, true>)); CARVE((k_cg_apply<true, false>));
 #undef CARVE
         }
+        if (getenv("SPH_BCARVE")) CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(getenv("SPH_BCARVE"))));
         CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (kMaxListCap + kStageExtra) * 64 * (kBlock / 32)));
         const int nf = s->c.nf, nb = s->c.nb;

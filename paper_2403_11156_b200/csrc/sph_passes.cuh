@@ -251,7 +251,9 @@ __device__ __forceinline__ float pair_gradf(const SimConst &c, float d2)
 //    stage[k * 32 + l]) and copied out as 32-bit words, one coalesced 128-byte row per warp store,
 //    instead of one partial-sector global store per entry.
 constexpr int kPosPad = 4;         // float4 elements readable past pos[nf - 1]
-constexpr int kStageExtra = 32;    // staging rows beyond kf (a run longer than this takes the guarded loop)
+constexpr int kStageExtra = 8;     // staging rows beyond kf.  Small on purpose: the builder's occupancy is set by this buffer
+                                   // (32 extra rows: 9 CTAs per SM, 207 us; 8: 10 CTAs, 198 us); a run that may not fit
+                                   // takes the guarded loop
 constexpr int kMaxListCap = 768;   // (kMaxListCap + kStageExtra) * 64 B * 4 warps <= 227 KB of shared memory
 
 __device__ __forceinline__ void sts_u16(uint32_t addr, int v)
