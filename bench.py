@@ -115,18 +115,18 @@ def kernel_work(name, nf_mean, nb_mean, cand_mean):
 
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the config-4 launches in the
-# committed `ncu --set full` capture profiles/r1d_ncu_full_summary.md (another run of the same command
+# committed `ncu --set full` capture profiles/r1e_ncu_full_summary.md (another run of the same command
 # as the roofline's timing: context for `achieved`, not a live measurement)
-NCU_PROFILE = "profiles/r1d_ncu_full_summary.md"
+NCU_PROFILE = "profiles/r1e_ncu_full_summary.md"
 NCU_TRAFFIC_BYTES = {
-    ("config4_splash_1p23M", "k_solver_p"): 129.498624e6 + 12.624128e6,
-    ("config4_splash_1p23M", "k_solver_c"): 149.176576e6 + 44.282368e6,
-    ("config4_splash_1p23M", "k_build_lists"): 26.509056e6 + 27.070976e6,
-    ("config4_splash_1p23M", "k_density_alpha"): 144.399616e6 + 31.389440e6,
+    ("config4_splash_1p23M", "k_solver_p"): 129.481984e6 + 4.196352e6,
+    ("config4_splash_1p23M", "k_solver_c"): 149.157376e6 + 28.326912e6,
+    ("config4_splash_1p23M", "k_build_lists"): 26.499072e6 + 27.364608e6,
+    ("config4_splash_1p23M", "k_density_alpha"): 144.392960e6 + 10.979072e6,
 }
 # l1tex__throughput.avg.pct_of_peak_sustained_active of the same capture: the list passes are bound by the
 # L1 gather path (see the profile), which is why their HBM fraction is low
-NCU_L1TEX_PCT = {"k_solver_p": 88.8, "k_solver_c": 86.8, "k_build_lists": 80.8, "k_density_alpha": 86.8}
+NCU_L1TEX_PCT = {"k_solver_p": 88.0, "k_solver_c": 85.5, "k_build_lists": 82.0, "k_density_alpha": 85.6}
 FINE_X = 2      # the library splits every grid cell into 2 slabs along x: x-runs cover 2.5 of the 3 cell widths
 
 
