@@ -599,3 +599,84 @@ def test_wcsph_vs_dfsph_centre_of_mass(oracle):
     c0 = sc.fluid_pos.astype(np.float64).mean(0)
     assert np.linalg.norm(ca - c0) > 0.25 * S * 0.2     # the fluid moved
     assert np.linalg.norm(ca - cb) <= 0.25 * S
+
+
+# ---------------------------------------------------------------- tests/golden fixtures
+
+def _golden():
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            name, val, _ = [t.strip() for t in line.split("|", 2)]
+            out[name] = float(val)
+    return out
+
+
+def test_golden_closed_forms_are_what_the_formulas_give():
+    """Every stored constant of tests/golden/closed_forms.txt is re-derived here in numpy from its
+    definition (no oracle involved), so a typo in the fixture cannot silently weaken a pin."""
+    g = _golden()
+    assert g["kernel_sigma_h3"] == pytest.approx(8.0 / np.pi, rel=1e-15)
+    a = 1 - 1 / np.sqrt(2); b = 1 - np.sqrt(3) / 2
+    assert g["akinci_volume_one_layer"] == pytest.approx(np.pi / (2 + 8 * a ** 3), abs=1e-6)
+    assert g["akinci_volume_two_layers"] == pytest.approx(np.pi / (2.25 + 16 * a ** 3 + 8 * b ** 3), abs=1e-6)
+
+    def w_and_wp(q):
+        if q <= 0.5:
+            return 6 * (q ** 3 - q ** 2) + 1, 6 * q * (3 * q - 2)
+        if q <= 1:
+            return 2 * (1 - q) ** 3, -6 * (1 - q) ** 2
+        return 0.0, 0.0
+
+    # lattice sums with h = 2 s, in units s = 1, sigma = 8 / (pi h^3)
+    h = 2.0
+    sigma = 8.0 / (np.pi * h ** 3)
+    rho = 0.0
+    T = 0.0
+    for i in range(-2, 3):
+        for j in range(-2, 3):
+            for k in range(-2, 3):
+                d = np.sqrt(i * i + j * j + k * k)
+                w, wp = w_and_wp(d / h)
+                rho += sigma * w
+                if d > 0:
+                    T += (sigma / h * wp) ** 2
+    assert g["lattice_density_over_rho0"] == pytest.approx(rho, abs=2e-8)
+    assert g["lattice_alpha_times_rho0_over_s2"] == pytest.approx(rho / T, rel=2e-6)
+
+    # Eq. 15 on v = (y^2, 0, 0), rho = rho0, m / rho = s^3 = 1
+    for key, ratio in (("laplacian_h_2s", 2), ("laplacian_h_4s", 4)):
+        h = float(ratio)
+        sigma = 8.0 / (np.pi * h ** 3)
+        n = ratio
+        lap = 0.0
+        for i in range(-n, n + 1):
+            for j in range(-n, n + 1):
+                for k in range(-n, n + 1):
+                    d2 = float(i * i + j * j + k * k)
+                    d = np.sqrt(d2)
+                    if d == 0 or d >= h:
+                        continue
+                    _, wp = w_and_wp(d / h)
+                    # particle i at the origin, neighbour at (i, j, k): x_ij = -(i, j, k), v_ij = (0 - j^2, 0, 0)
+                    vij_dot_xij = (-(j * j)) * (-i)
+                    gradx = sigma / h * wp * (-i) / d
+                    lap += 10.0 * vij_dot_xij / (d2 + 0.01 * h * h) * gradx
+        assert g[key] == pytest.approx(lap, abs=2e-6), (key, lap)
+
+
+def test_oracle_matches_golden_lattice_constants(oracle):
+    g = _golden()
+    n = 9
+    gr = (np.arange(n) + 0.5) * S
+    z, y, x = np.meshgrid(gr, gr, gr, indexing="ij")
+    pos = np.stack([x.ravel(), y.ravel(), z.ravel()], 1)
+    sim = make_sim(oracle, np.zeros((n ** 3, 3), dtype=np.float32))
+    sim.set_state(pos, np.zeros_like(pos))
+    sim.build_grid(); sim.compute_density_alpha()
+    c = (n // 2) * (n * n + n + 1)
+    assert sim.density()[c] / RHO0 == pytest.approx(g["lattice_density_over_rho0"], abs=2e-8)
+    assert sim.alpha()[c] * RHO0 / S ** 2 == pytest.approx(g["lattice_alpha_times_rho0_over_s2"], rel=2e-6)
