@@ -60,7 +60,8 @@ struct SphSim {
     uint16_t *nl_f = nullptr;       // 16-bit (run, offset) entries, warp-tiled (sph_passes.cuh)
     int *nl_b = nullptr, *ncount = nullptr;
     float *partial = nullptr, *partial2 = nullptr;
-    float4 *cg_r = nullptr, *cg_p = nullptr, *cg_Ap = nullptr;
+    float4 *cg_r = nullptr, *cg_Ap = nullptr;
+    PV *cg_p = nullptr;             // search direction as {x | p, rho} records (gathered by k_cg_apply)
     // boundary store
     float4 *borig_pos = nullptr, *borig_vel = nullptr, *brest = nullptr, *bforce = nullptr;
     float4 *bpos_s = nullptr, *bvel_s = nullptr;
@@ -217,7 +218,7 @@ size_t layout(SphSim &s, void *base)
     s.partial = w.take<float>((size_t)s.nblocks);
     s.partial2 = w.take<float>((size_t)s.nblocks);
     if (s.prm.viscosity_mode == 2) {
-        s.cg_r = w.take<float4>(nf1); s.cg_p = w.take<float4>(nf1); s.cg_Ap = w.take<float4>(nf1);
+        s.cg_r = w.take<float4>(nf1); s.cg_p = w.take<PV>(nf1); s.cg_Ap = w.take<float4>(nf1);
     }
     s.borig_pos = w.take<float4>(nb1); s.borig_vel = w.take<float4>(nb1);
     s.brest = w.take<float4>(nb1); s.bforce = w.take<float4>(nb1);
@@ -463,7 +464,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
                         return (int)SPH_OK;
                     },
                     [&](const LoopCtx &lc) -> int {
-                        LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, s->cg_p, s->cg_Ap, (float4 *)nullptr, s->partial, (float *)nullptr);
+                        LAUNCH(s, (k_cg_apply<LIST, false>), s->nblocks, kBlock, lc.st, p, reinterpret_cast<const float4 *>(s->cg_p), s->cg_Ap, (PV *)nullptr, s->partial, (float *)nullptr);
                         LAUNCH(s, k_cg_ctrl1, 1, kCtrlThreads, lc.st, s->partial, s->nblocks, s->ctl);
                         LAUNCH(s, k_cg_update, cdiv(nf, 256), 256, lc.st, nf, s->ctl, s->cg_p, s->cg_Ap, s->pvB, s->cg_r, s->partial2);
                         LAUNCH(s, k_cg_ctrl2, 1, kCtrlThreads, lc.st, s->partial2, cdiv(nf, 256), s->ctl, s->stats, lc.h, lc.use_handle);

@@ -751,13 +751,14 @@ k_explicit_viscosity(PassCtx p, const PV *__restrict__ vin, PV *__restrict__ vou
 // A11: implicit viscosity (Eq. 16-19; R4, R21, R23), matrix-free CG on
 // (I - dt A) v* = v~ with
 //   (A u)_i = 2(d+2) sum_j mu m / (rho_i rho_j) (u_ij.x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij.
-// Vectors are float4 with rho in .w (the start vector b = v~ lives in the PV records).  out_i = u_i - dt (A u)_i when RESIDUAL0 = false;
+// Vectors are float4 with rho in .w; the two that are gathered -- the start vector b = v~ and the search
+// direction p -- live in 32-byte {x | vector} records (one 256-bit gather per neighbour).  out_i = u_i - dt (A u)_i when RESIDUAL0 = false;
 // RESIDUAL0 = true is the start-up r0 = b - (I - dt A) b = dt A b (x0 = b = v~), which also seeds
 // the search direction and reduces |b|^2, |r0|^2.
 template <bool LIST, bool RESIDUAL0>
 __global__ void __launch_bounds__(kBlock)
-k_cg_apply(PassCtx p, const float4 *__restrict__ u /* RESIDUAL0: PV records */, float4 *__restrict__ out,
-           float4 *__restrict__ out2, float *__restrict__ partial, float *__restrict__ partial2)
+k_cg_apply(PassCtx p, const float4 *__restrict__ u /* PV records: velocities (RESIDUAL0) or search direction */,
+           float4 *__restrict__ out, PV *__restrict__ out2, float *__restrict__ partial, float *__restrict__ partial2)
 {
     __shared__ float red[kBlock / 32];
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
@@ -766,9 +767,9 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u /* RESIDUAL0: PV records */, 
     float t1 = 0.f, t2 = 0.f;
     if (i < c.nf) {
         float4 xi = p.pos[i];
-        float4 ui = RESIDUAL0 ? u[2 * i + 1] : u[i];
+        float4 ui = u[2 * i + 1];
         float ax = 0.f, ay = 0.f, az = 0.f;
-        for_each_neighbor<LIST, false, RESIDUAL0 ? 3 : 2, !RESIDUAL0>(p, RESIDUAL0 ? u : p.pos, u, tbl, i, xi.x, xi.y, xi.z,
+        for_each_neighbor<LIST, false, 3, false>(p, u, nullptr, tbl, i, xi.x, xi.y, xi.z,
             [&](int, float4, float4 uj, float dx, float dy, float dz, float d2) {
                 float du = fmaf(ui.x - uj.x, dx, fmaf(ui.y - uj.y, dy, (ui.z - uj.z) * dz));
                 float s = pair_gradf(c, d2) * du / ((d2 + c.visc_eps) * uj.w);
@@ -780,7 +781,7 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u /* RESIDUAL0: PV records */, 
         if (RESIDUAL0) {
             float4 r = make_float4(Ax, Ay, Az, ui.w);
             out[i] = r;                                            // r0
-            out2[i] = r;                                           // p0 = r0
+            out2[i].x = xi; out2[i].v = r;                         // p0 = r0 (a record: the next applies gather it)
             t1 = fmaf(ui.x, ui.x, fmaf(ui.y, ui.y, ui.z * ui.z));  // |b|^2
             t2 = fmaf(Ax, Ax, fmaf(Ay, Ay, Az * Az));              // |r0|^2
         } else {
@@ -799,7 +800,7 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u /* RESIDUAL0: PV records */, 
 
 // x += a p;  r -= a Ap;  partial |r|^2
 __global__ void __launch_bounds__(256)
-k_cg_update(int n, const DevControl *__restrict__ ctl, const float4 *__restrict__ pd,
+k_cg_update(int n, const DevControl *__restrict__ ctl, const PV *__restrict__ pd,
             const float4 *__restrict__ Ap, PV *__restrict__ x, float4 *__restrict__ r,
             float *__restrict__ partial)
 {
@@ -808,7 +809,7 @@ k_cg_update(int n, const DevControl *__restrict__ ctl, const float4 *__restrict_
     float t = 0.f;
     if (i < n) {
         float a = (float)ctl->cg_alpha;
-        float4 pv = pd[i], av = Ap[i], xv = x[i].v, rv = r[i];
+        float4 pv = pd[i].v, av = Ap[i], xv = x[i].v, rv = r[i];
         xv.x = fmaf(a, pv.x, xv.x); xv.y = fmaf(a, pv.y, xv.y); xv.z = fmaf(a, pv.z, xv.z);
         rv.x = fmaf(-a, av.x, rv.x); rv.y = fmaf(-a, av.y, rv.y); rv.z = fmaf(-a, av.z, rv.z);
         x[i].v = xv; r[i] = rv;
@@ -821,14 +822,14 @@ k_cg_update(int n, const DevControl *__restrict__ ctl, const float4 *__restrict_
 // p = r + beta p
 __global__ void __launch_bounds__(256)
 k_cg_direction(int n, const DevControl *__restrict__ ctl, const float4 *__restrict__ r,
-               float4 *__restrict__ pd)
+               PV *__restrict__ pd)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float b = (float)ctl->cg_beta;
-    float4 rv = r[i], pv = pd[i];
+    float4 rv = r[i], pv = pd[i].v;
     pv.x = fmaf(b, pv.x, rv.x); pv.y = fmaf(b, pv.y, rv.y); pv.z = fmaf(b, pv.z, rv.z);
-    pd[i] = pv;
+    pd[i].v = pv;
 }
 
 // ---------------------------------------------------------------------------------------------
