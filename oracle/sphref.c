@@ -56,6 +56,8 @@ typedef struct SphRefParams {
     int enable_divergence_solve;
     int force_iterations;
     double wcsph_stiffness, wcsph_exponent;
+    double cfl_factor;          /* lambda of reading R26; 0 => fixed dt */
+    double dt_min;
 } SphRefParams;
 
 typedef struct SphRefBody {
@@ -68,6 +70,7 @@ typedef struct SphRefBody {
 typedef struct SphRefStats {
     int it_v, it_d, cg_iters, oob_count;
     double err_v, err_rho, cg_residual, v_max;
+    double dt_last, sim_time;   /* time step of the last step, simulated time so far */
 } SphRefStats;
 
 /* cell list over an arbitrary point set (reading R11) */
@@ -97,6 +100,7 @@ typedef struct SphRef {
     int *nb_start, *nb_idx; /* CSR boundary neighbours of fluid i */
     int lists_valid;
     SphRefStats stats;
+    double dt_max, forced_dt;   /* configured dt (upper bound of the CFL rule); > 0: dt imposed by the caller */
     double *cg_hist; int cg_hist_n;
 } SphRef;
 
@@ -330,6 +334,7 @@ SphRef *sphref_create(const SphRefParams *p, int nf, const float *fpos, const fl
 {
     SphRef *s = (SphRef *)calloc(1, sizeof(SphRef));
     s->p = *p;
+    s->dt_max = p->dt; s->forced_dt = 0.0;
     s->nf = nf; s->nb = nb; s->nbodies = nbodies;
     double d = 2.0 * p->particle_radius;
     s->m = p->particle_mass > 0.0 ? p->particle_mass : p->rest_density * d * d * d; /* R3 */
@@ -698,6 +703,26 @@ static double max_speed(const SphRef *s)
     return sqrt(vm);
 }
 
+/* Time step of the coming step (reading R26; PAPER.md:49 only says that implicit pressure solvers allow
+ * "larger time steps", the rule is the usual CFL condition of the cited DFSPH source [5]):
+ *   dt = clamp(lambda 2r / max_i |v_i|, dt_min, dt_max), dt_max = the configured dt, lambda = cfl_factor,
+ * with the velocities at the START of the step; lambda = 0 keeps dt fixed.  forced_dt > 0 overrides
+ * (parity runs hand the GPU's fp32 choice to the oracle, as they do with the iteration counts, R20). */
+static double choose_dt(SphRef *s)
+{
+    const SphRefParams *p = &s->p;
+    double dt = s->dt_max;
+    if (s->forced_dt > 0.0) return s->forced_dt;
+    if (p->cfl_factor > 0.0) {
+        double vm = max_speed(s);
+        double c = p->cfl_factor * 2.0 * p->particle_radius / (vm > 1e-30 ? vm : 1e-30);
+        if (c < dt) dt = c;
+        if (dt < p->dt_min) dt = p->dt_min;
+    }
+    return dt;
+}
+void sphref_set_forced_dt(SphRef *s, double dt) { s->forced_dt = dt; }
+
 /* One DFSPH step, (c.2) steps 1-7 (Alg. 1 PAPER.md:127-134 with the pressure solve of
  * Alg. 2 realised by DFSPH [5]; order of stages per PAPER.md:262 and reading R13).
  * forced_*: -1 = free running (tolerances decide), >= 0 = exactly that many iterations. */
@@ -705,6 +730,7 @@ int sphref_step_dfsph(SphRef *s, int forced_v, int forced_d, int forced_cg)
 {
     const SphRefParams *p = &s->p;
     int n3 = 3 * s->nf;
+    s->p.dt = choose_dt(s);                                 /* every stage below reads p->dt */
     if (p->force_iterations) {
         if (forced_v < 0) forced_v = p->min_iter_divergence;
         if (forced_d < 0) forced_d = p->min_iter_density;
@@ -729,6 +755,8 @@ int sphref_step_dfsph(SphRef *s, int forced_v, int forced_d, int forced_cg)
     for (int i = 0; i < n3; ++i) s->x[i] += p->dt * s->v[i]; /* 6: symplectic Euler, Alg. 1 l.5-6 */
     sphref_rigid_step(s);                                   /* 7 */
     s->stats.v_max = max_speed(s);
+    s->stats.dt_last = s->p.dt; s->stats.sim_time += s->p.dt;
+    s->p.dt = s->dt_max;
     s->lists_valid = 0;
     return 0;
 }
@@ -742,6 +770,7 @@ int sphref_step_wcsph(SphRef *s)
     const SphRefParams *p = &s->p;
     int n3 = 3 * s->nf;
     double h = p->support_radius, m = s->m;
+    s->p.dt = choose_dt(s);
     sphref_build_grid(s);
     memset(s->bforce, 0, sizeof(double) * 3 * (size_t)(s->nb > 0 ? s->nb : 1));
     sphref_compute_density_alpha(s);
@@ -760,6 +789,8 @@ int sphref_step_wcsph(SphRef *s)
     for (int i = 0; i < n3; ++i) s->x[i] += p->dt * s->v[i];
     sphref_rigid_step(s);
     s->stats.it_v = 0; s->stats.it_d = 0; s->stats.v_max = max_speed(s);
+    s->stats.dt_last = s->p.dt; s->stats.sim_time += s->p.dt;
+    s->p.dt = s->dt_max;
     free(rt); free(acc);
     s->lists_valid = 0;
     return 0;
@@ -786,7 +817,7 @@ void sphref_set_boundary_state(SphRef *s, const float *bpos, const float *bvel)
 }
 void sphref_set_bodies(SphRef *s, const SphRefBody *b) { for (int i = 0; i < s->nbodies; ++i) s->bodies[i] = b[i]; }
 void sphref_get_bodies(const SphRef *s, SphRefBody *b) { for (int i = 0; i < s->nbodies; ++i) b[i] = s->bodies[i]; }
-void sphref_set_params(SphRef *s, const SphRefParams *p) { s->p = *p; }
+void sphref_set_params(SphRef *s, const SphRefParams *p) { s->p = *p; s->dt_max = p->dt; }
 
 double *sphref_pos(SphRef *s) { return s->x; }
 double *sphref_vel(SphRef *s) { return s->v; }

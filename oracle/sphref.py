@@ -41,6 +41,7 @@ class Params(C.Structure):
         ("eta_divergence", C.c_double), ("min_iter_divergence", C.c_int), ("max_iter_divergence", C.c_int),
         ("enable_divergence_solve", C.c_int), ("force_iterations", C.c_int),
         ("wcsph_stiffness", C.c_double), ("wcsph_exponent", C.c_double),
+        ("cfl_factor", C.c_double), ("dt_min", C.c_double),
     ]
 
 
@@ -57,7 +58,7 @@ class Body(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("it_v", C.c_int), ("it_d", C.c_int), ("cg_iters", C.c_int), ("oob_count", C.c_int),
                 ("err_v", C.c_double), ("err_rho", C.c_double), ("cg_residual", C.c_double),
-                ("v_max", C.c_double)]
+                ("v_max", C.c_double), ("dt_last", C.c_double), ("sim_time", C.c_double)]
 
 
 _lib = None
@@ -72,6 +73,8 @@ def lib():
         L.sphref_create.restype = C.c_void_p
         L.sphref_create.argtypes = [C.POINTER(Params), C.c_int, C.c_void_p, C.c_void_p, C.c_int,
                                     C.c_void_p, C.c_void_p, C.c_int, C.POINTER(Body)]
+        L.sphref_set_forced_dt.argtypes = [C.c_void_p, C.c_double]
+        L.sphref_set_forced_dt.restype = None
         L.sphref_destroy.argtypes = [C.c_void_p]
         for name in ("sphref_build_grid", "sphref_compute_density_alpha", "sphref_step_wcsph"):
             getattr(L, name).argtypes = [C.c_void_p]
@@ -130,7 +133,7 @@ def num_threads() -> int:
 def make_params(prm: Dict[str, object]) -> Params:
     p = Params()
     for name, ctype in Params._fields_:
-        val = prm[name]
+        val = prm.get(name, 0.0) if name in ("cfl_factor", "dt_min") else prm[name]
         if hasattr(ctype, "_length_"):
             setattr(p, name, ctype(*[float(v) for v in val]))
         else:
@@ -210,6 +213,11 @@ class Sim:
 
     def step_wcsph(self):
         lib().sphref_step_wcsph(self._h)
+
+    def set_forced_dt(self, dt: float = 0.0):
+        """dt > 0: every following step uses exactly this time step (parity runs hand over the GPU's
+        choice); 0: the CFL rule of reading R26 decides (fixed dt when cfl_factor = 0)."""
+        lib().sphref_set_forced_dt(self._h, float(dt))
 
     def _solve(self, fn, vel, forced):
         v = np.ascontiguousarray(vel, dtype=np.float64).copy()

@@ -180,6 +180,8 @@ def default_params(r: float, dt: float) -> Dict[str, object]:
         force_iterations=0,
         wcsph_stiffness=50000.0,
         wcsph_exponent=7.0,
+        cfl_factor=0.0,                       # 0 => fixed dt (all BASELINE configs); > 0: CFL-adaptive dt, reading R26
+        dt_min=0.0,
     )
 
 

@@ -680,3 +680,52 @@ def test_oracle_matches_golden_lattice_constants(oracle):
     c = (n // 2) * (n * n + n + 1)
     assert sim.density()[c] / RHO0 == pytest.approx(g["lattice_density_over_rho0"], abs=2e-8)
     assert sim.alpha()[c] * RHO0 / S ** 2 == pytest.approx(g["lattice_alpha_times_rho0_over_s2"], rel=2e-6)
+
+
+# ---------------------------------------------------------------- CFL-adaptive time step (R26, NEXT-1)
+
+def test_cfl_time_step_rule_and_free_fall_recurrence(oracle):
+    """dt_n = clamp(lambda 2r / max|v|, dt_min, dt_max) with the velocities at the start of step n.
+    A block in free fall far from everything feels no pressure (rho* <= rho0), so v and x follow
+    the symplectic-Euler recurrence with the VARIABLE dt -- re-evaluated here in plain Python.
+    Catches: v_max taken after instead of before the step, clamp order, dt not used consistently
+    by gravity and integration."""
+    lam, dt_max, dt_min = 0.4, 4e-4, 1e-5
+    g = 9.81
+    n = 4
+    gr = (np.arange(n) + 0.5) * S
+    z, y, x = np.meshgrid(gr, gr, gr, indexing="ij")
+    pos = np.stack([x.ravel(), y.ravel(), z.ravel() + 5.0], 1)
+    v0 = np.tile(np.array([[3.0, 0.0, -19.5]]), (len(pos), 1))    # |v| crosses lambda 2r / dt_max = 20 m/s on the way
+    sim = make_sim(oracle, pos.astype(np.float32), v0.astype(np.float32), cfl_factor=lam, dt_min=dt_min,
+                   domain_min=(-1.0, -1.0, 0.0), domain_max=(2.0, 1.0, 6.0))
+    p0 = sim.pos().copy()
+    v = np.array([3.0, 0.0, -19.5])
+    xx = np.zeros(3)
+    t = 0.0
+    dts = []
+    for k in range(200):
+        dt = min(dt_max, max(dt_min, lam * 2 * R / np.linalg.norm(v)))
+        dts.append(dt)
+        sim.step_dfsph()
+        st = sim.stats()
+        assert st["dt_last"] == pytest.approx(dt, rel=1e-12), k
+        v = v + dt * np.array([0.0, 0.0, -g])
+        xx = xx + dt * v
+        t += dt
+        assert st["sim_time"] == pytest.approx(t, rel=1e-12)
+    assert dts[0] == dt_max and dts[-1] < dt_max         # the rule switched on during the fall
+    assert np.allclose(sim.vel(), v[None, :], rtol=1e-12, atol=1e-12)
+    assert np.allclose(sim.pos() - p0, xx[None, :], rtol=1e-10, atol=1e-12)
+    # clamps: slow fluid -> dt_max; forced dt overrides; lambda = 0 -> fixed dt
+    sim.set_state(p0, np.full_like(p0, 1e-3)); sim.step_dfsph()
+    assert sim.stats()["dt_last"] == dt_max
+    sim.set_state(p0, np.tile(np.array([[1e4, 0.0, 0.0]]), (len(p0), 1))); sim.step_dfsph()
+    assert sim.stats()["dt_last"] == dt_min
+    sim.set_forced_dt(1.25e-4); sim.step_dfsph()
+    assert sim.stats()["dt_last"] == 1.25e-4
+    sim.set_forced_dt(0.0)
+    fixed = make_sim(oracle, pos.astype(np.float32), (10 * v0).astype(np.float32),
+                     domain_min=(-1.0, -1.0, 0.0), domain_max=(2.0, 1.0, 6.0))
+    fixed.step_dfsph()
+    assert fixed.stats()["dt_last"] == 4e-4
