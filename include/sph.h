@@ -54,7 +54,7 @@ typedef struct SphParams {
     float support_radius;      /* h, support radius of W (= 4r) */
     float rest_density;        /* rho0 */
     float particle_mass;       /* 0 => rho0 (2r)^3                    reading R3 */
-    float dt;                  /* fixed time step                     reading R19 */
+    float dt;                  /* time step; with cfl_factor > 0 its upper bound   readings R19, R26 */
     float gravity[3];
     float domain_min[3];       /* grid origin and extent; particles outside are clamped into */
     float domain_max[3];       /*   the edge cells and counted in SphStats.oob_count (R11)   */
@@ -81,6 +81,10 @@ typedef struct SphParams {
                                   path); 0: plain launches, loop predicates read by the host */
     int   use_neighbor_list;   /* 1: solver passes gather through the per-step neighbour list
                                   (default); 0: every pass re-walks the 27 cells */
+    float cfl_factor;          /* lambda > 0: CFL-adaptive step, evaluated on the device before every step,
+                                  dt = clamp(lambda 2r / max_i |v_i|, dt_min, dt) with the velocities at the
+                                  step's start (reading R26); 0: fixed dt */
+    float dt_min;
 } SphParams;
 
 /* Rigid body = contiguous range of boundary samples (Akinci [3]).  Dynamics are
@@ -124,6 +128,8 @@ typedef struct SphStats {
     int   max_fluid_neighbors;   /* largest fluid / boundary neighbour count seen in the last list build */
     int   max_boundary_neighbors;
     float mean_fluid_neighbors;
+    float dt_last;               /* time step of the last step */
+    double sim_time;             /* simulated time since create (sum of the steps' dt) */
 } SphStats;
 
 /* Fields of sph_read_state / sph_write_state.  Per-particle fields are in ORIGINAL id order. */

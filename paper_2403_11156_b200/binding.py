@@ -43,6 +43,7 @@ class SphParams(C.Structure):
         ("wcsph_stiffness", C.c_float), ("wcsph_exponent", C.c_float),
         ("max_fluid_neighbors", C.c_int), ("max_boundary_neighbors", C.c_int),
         ("use_cuda_graph", C.c_int), ("use_neighbor_list", C.c_int),
+        ("cfl_factor", C.c_float), ("dt_min", C.c_float),
     ]
 
 
@@ -71,7 +72,7 @@ class SphStats(C.Structure):
         ("oob_count", C.c_int), ("overflow_count", C.c_int), ("nan_count", C.c_int),
         ("max_iter_hit", C.c_int), ("v_max", C.c_float),
         ("max_fluid_neighbors", C.c_int), ("max_boundary_neighbors", C.c_int),
-        ("mean_fluid_neighbors", C.c_float),
+        ("mean_fluid_neighbors", C.c_float), ("dt_last", C.c_float), ("sim_time", C.c_double),
     ]
 
 
@@ -121,7 +122,8 @@ def load() -> C.CDLL:
 def make_params(prm: Dict[str, object]) -> SphParams:
     """dict (keys of scenes.default_params + optional library switches) -> SphParams."""
     p = SphParams()
-    defaults = dict(max_fluid_neighbors=0, max_boundary_neighbors=0, use_cuda_graph=1, use_neighbor_list=1)
+    defaults = dict(max_fluid_neighbors=0, max_boundary_neighbors=0, use_cuda_graph=1, use_neighbor_list=1,
+                    cfl_factor=0.0, dt_min=0.0)
     for name, ctype in SphParams._fields_:
         val = prm.get(name, defaults.get(name))
         if val is None:

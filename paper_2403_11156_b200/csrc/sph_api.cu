@@ -73,6 +73,7 @@ struct SphSim {
     size_t staging_bytes = 0;
     // host
     int *pinned = nullptr;          // small pinned block (loop predicate, stats)
+    bool vmax_valid = false;        // stats->vmax_bits = max |v| of the persistent store (needed by the CFL rule)
     bool derived_valid = false;     // B-order fields (rho, alpha, lists, cell_start) match the store
     cudaGraphExec_t exec[2] = { nullptr, nullptr };   // 0 DFSPH, 1 WCSPH
     long long fixed_nodes[2] = { 0, 0 };
@@ -166,6 +167,9 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     if (nf < 0 || nb < 0) { why = "negative particle count"; return false; }
     if (!(p.particle_radius > 0.f) || !(p.rest_density > 0.f) || !(p.dt > 0.f)) {
         why = "particle_radius, rest_density and dt must be > 0"; return false;
+    }
+    if (!(p.cfl_factor >= 0.f) || !(p.dt_min >= 0.f) || p.dt_min > p.dt) {
+        why = "cfl_factor must be >= 0 and 0 <= dt_min <= dt"; return false;
     }
     if (!make_geom(p, c.g, why)) return false;
     c.nf = nf; c.nb = nb;
@@ -428,7 +432,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
     const int nf = s->c.nf;
     const bool dyn = s->c.has_dynamic != 0;
     long long *bc = s->body_nodes[method];
-    LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl);
+    LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl, s->prm.cfl_factor * 2.0f * s->prm.particle_radius, s->prm.dt_min, s->prm.dt);
     if (dyn) {
         int rc = enqueue_boundary_grid(s, st);
         if (rc) return rc;
@@ -496,7 +500,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
         LAUNCH(s, k_rigid_step, s->nbodies, 256, st, s->c, s->bodies, s->prm.tank_min[0], s->prm.tank_min[1],
                s->prm.tank_min[2], s->prm.tank_max[0], s->prm.tank_max[1], s->prm.tank_max[2], s->brest, s->bforce,
                s->borig_pos, s->borig_vel);
-    LAUNCH(s, k_step_end, 1, 1, st, s->stats);
+    LAUNCH(s, k_step_end, 1, 1, st, s->stats, s->ctl);
     return SPH_OK;
 }
 
@@ -533,6 +537,12 @@ int do_steps(SphSim *s, int method, int n_steps)
     if (!s) return SPH_EINVAL;
     if (n_steps < 0) { s->err = "n_steps < 0"; return SPH_EINVAL; }
     DeviceGuard dg(s->device);
+    if (s->prm.cfl_factor > 0.f && !s->vmax_valid && n_steps > 0 && s->c.nf > 0) {
+        // the CFL rule needs max |v| at the start of the step; later steps get it from the integration tail
+        CUDA_TRY(s, cudaMemsetAsync(&s->stats->vmax_bits, 0, sizeof(unsigned), s->stream));
+        LAUNCH(s, k_vmax, cdiv(s->c.nf, 256), 256, s->stream, s->velA, s->c.nf, &s->stats->vmax_bits);
+    }
+    if (n_steps > 0) s->vmax_valid = true;
     if (s->prm.use_cuda_graph) {
         if (!s->exec[method]) {
             int rc = build_graph(s, method);
@@ -618,7 +628,7 @@ int import_field(SphSim *s, int field, const void *src, size_t bytes)
     if (bytes == 0) return SPH_OK;
     switch (field) {
     case SPH_FIELD_POS: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->posA); break;
-    case SPH_FIELD_VEL: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->velA); break;
+    case SPH_FIELD_VEL: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->velA); s->vmax_valid = false; break;
     case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_pos); break;
     case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_vel); break;
     case SPH_FIELD_RIGID_BODIES:
@@ -690,6 +700,7 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
     }
     if ((reinterpret_cast<uintptr_t>(buf->workspace) & 255) != 0) { s->err = "workspace must be 256-byte aligned"; return fail(SPH_EINVAL); }
     layout(*s, buf->workspace);
+    s->c.dt_dev = &s->ctl->dt;
 
     DeviceGuard dg(s->device);
     auto run = [&]() -> int {
@@ -726,6 +737,7 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
         hc.min_v = p.min_iter_divergence; hc.max_v = p.max_iter_divergence;
         hc.min_d = p.min_iter_density; hc.max_d = p.max_iter_density;
         hc.max_cg = p.cg_max_iter; hc.enable_div = p.enable_divergence_solve;
+        hc.dt = p.dt;
         hc.eta_v = p.eta_divergence; hc.eta_d = p.eta_density; hc.cg_tol = p.cg_rel_tol;
         memcpy(s->pinned, &hc, sizeof hc);
         CUDA_TRY(s, cudaMemcpyAsync(s->ctl, s->pinned, sizeof hc, cudaMemcpyHostToDevice, st));
@@ -867,6 +879,7 @@ int sph_read_stats(SphSim *s, SphStats *o)
     o->err_v = h->err_v; o->err_rho = h->err_rho; o->cg_residual = h->cg_residual;
     o->oob_count = h->oob; o->overflow_count = h->lc.overflow; o->nan_count = h->nan_count;
     o->max_iter_hit = h->max_iter_hit;
+    o->dt_last = h->dt_last; o->sim_time = h->sim_time;
     unsigned vb = h->vmax_bits; float vm; memcpy(&vm, &vb, 4); o->v_max = vm;
     o->max_fluid_neighbors = h->lc.max_f; o->max_boundary_neighbors = h->lc.max_b;
     o->mean_fluid_neighbors = s->c.nf > 0 ? (float)((double)h->lc.sum_f / (double)s->c.nf) : 0.f;

@@ -41,7 +41,8 @@ struct SimConst {
     float ga, gb;        // gradient factor of the inner branch: 6 (3q - 2) / h = ga r + gb, ga = 18 / h^2, gb = -12 / h
     float half_h;        // branch point q = 1/2 in terms of r
     float m;             // fluid particle mass     (R3)
-    float rho0, dt;
+    float rho0, dt;      // dt: the configured step (upper bound of the CFL rule, reading R26)
+    const float *dt_dev; // the CURRENT step's dt (DevControl::dt), chosen on the device by k_step_begin
     float gx, gy, gz;
     float nu, mu;        // kinematic / dynamic viscosity (mu = nu rho0, R21)
     float visc_eps;      // 0.01 h^2                (Eq. 15 / 19, R4)
@@ -61,6 +62,7 @@ struct DevControl {
     int it;                              // iteration counter of the running loop
     double cg_bb, cg_rr, cg_alpha, cg_beta;
     int cg_break;
+    float dt;                            // time step of the running step (R26; = SphParams.dt when cfl_factor = 0)
     unsigned long long acc;              // running P-pass: CTA counter (top 20 bits) | fixed-point error sum (A12)
 };
 
@@ -76,7 +78,12 @@ struct DevStats {
     int oob, nan_count;
     unsigned vmax_bits;
     ListCounters lc;
+    float dt_last;
+    double sim_time;
 };
+
+// time step of the running step
+__device__ __forceinline__ float step_dt(const SimConst &c) { return __ldg(c.dt_dev); }
 
 // ---------------------------------------------------------------------------------------------
 // Cell coordinate of one point: (int)floorf((x - o) * inv_c) with separate fp32 subtract and

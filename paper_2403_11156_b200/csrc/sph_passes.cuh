@@ -488,7 +488,7 @@ __device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevCo
     __shared__ float red[kBlock / 32];
     float s = block_sum(term, red);
     if (threadIdx.x != 0) return;
-    const double norm = MODE == MODE_DIV ? (double)c.dt / (double)c.rho0 : 1.0 / (double)c.rho0;
+    const double norm = MODE == MODE_DIV ? (double)step_dt(c) / (double)c.rho0 : 1.0 / (double)c.rho0;
     const unsigned long long cap = ((1ull << kAccSumBits) - 1ull) / (unsigned long long)gridDim.x;
     double d = (double)s * norm * (double)(1u << kAccFracBits) + 0.5;
     unsigned long long q = d > 0.0 ? (d < (double)cap ? (unsigned long long)d : cap) : 0ull;   // NaN -> 0
@@ -568,7 +568,7 @@ k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
             bool on = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;
             float D = c.grad_c * fmaf(c.m, df, db);
             term = fmaxf(D, 0.f);
-            float kappa = a * term / c.dt;
+            float kappa = a * term / step_dt(c);
             posk[i] = make_float4(xi.x, xi.y, xi.z, on ? kappa / rho : 0.f);
         }
     }
@@ -613,13 +613,14 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
                 db = fmaf(gf, dv, db);
             });
         float D = c.grad_c * fmaf(c.m, df, db);
+        const float dt = step_dt(c);
         float rho = vi.w, a = alpha[i], kappa;
         if (MODE == MODE_DIV) {
             term = fmaxf(D, 0.f);
-            kappa = a * term / c.dt;
+            kappa = a * term / dt;
         } else {
-            term = fmaxf(fmaf(c.dt, D, rho), c.rho0) - c.rho0;
-            kappa = a * term / (c.dt * c.dt);
+            term = fmaxf(fmaf(dt, D, rho), c.rho0) - c.rho0;
+            kappa = a * term / (dt * dt);
             // the P-pass that opens the density loop runs even when the loop is switched off
             // (forced 0 iterations): kappa = 0 then, and its C-pass only integrates
             if (first && !(ctl->forced_d != 0 && ctl->max_d > 0)) kappa = 0.f;
@@ -674,23 +675,24 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, PV *__restrict__ pv, CTai
                 bx = fmaf(s, dx, bx); by = fmaf(s, dy, by); bz = fmaf(s, dz, bz);
             });
         float4 v = pv[i].v;
+        const float dt = step_dt(c);
         if (TAIL == TAIL_WCSPH && t.add_gravity) {              // A10: v + dt g first, then the pressure term
-            v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
+            v.x = fmaf(dt, c.gx, v.x); v.y = fmaf(dt, c.gy, v.y); v.z = fmaf(dt, c.gz, v.z);
         }
-        float k = c.dt * c.grad_c;
+        float k = dt * c.grad_c;
         v.x -= k * fmaf(c.m, fx, kri * bx);
         v.y -= k * fmaf(c.m, fy, kri * by);
         v.z -= k * fmaf(c.m, fz, kri * bz);
         if (TAIL == TAIL_DIV) {
             if (last && t.add_gravity) {
-                v.x = fmaf(c.dt, c.gx, v.x); v.y = fmaf(c.dt, c.gy, v.y); v.z = fmaf(c.dt, c.gz, v.z);
+                v.x = fmaf(dt, c.gx, v.x); v.y = fmaf(dt, c.gy, v.y); v.z = fmaf(dt, c.gz, v.z);
             }
             pv[i].v = v;
         } else {
             pv[i].v = v;
             if (last) {
                 float4 x;
-                x.x = fmaf(c.dt, v.x, xi.x); x.y = fmaf(c.dt, v.y, xi.y); x.z = fmaf(c.dt, v.z, xi.z);
+                x.x = fmaf(dt, v.x, xi.x); x.y = fmaf(dt, v.y, xi.y); x.z = fmaf(dt, v.z, xi.z);
                 x.w = 0.f;
                 t.pos_out[i] = x;
                 t.vel_out[i] = make_float4(v.x, v.y, v.z, 0.f);
@@ -739,10 +741,11 @@ k_explicit_viscosity(PassCtx p, const PV *__restrict__ vin, PV *__restrict__ vou
             ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay); az = fmaf(s, dz, az);
         },
         [&](int, float4, float, float, float, float) {});
-    float k = c.dt * c.nu * 10.0f * c.m * c.grad_c;
-    vi.x += fmaf(c.dt, c.gx, k * ax);
-    vi.y += fmaf(c.dt, c.gy, k * ay);
-    vi.z += fmaf(c.dt, c.gz, k * az);
+    const float dt = step_dt(c);
+    float k = dt * c.nu * 10.0f * c.m * c.grad_c;
+    vi.x += fmaf(dt, c.gx, k * ax);
+    vi.y += fmaf(dt, c.gy, k * ay);
+    vi.z += fmaf(dt, c.gz, k * az);
     vout[i].x = xi;
     vout[i].v = vi;
 }
@@ -776,7 +779,7 @@ k_cg_apply(PassCtx p, const float4 *__restrict__ u /* PV records: velocities (RE
                 ax = fmaf(s, dx, ax); ay = fmaf(s, dy, ay); az = fmaf(s, dz, az);
             },
             [&](int, float4, float, float, float, float) {});
-        float k = c.dt * 10.0f * c.mu * c.m * c.grad_c / ui.w;     // dt * 2(d+2) mu m / rho_i
+        float k = step_dt(c) * 10.0f * c.mu * c.m * c.grad_c / ui.w;   // dt * 2(d+2) mu m / rho_i
         float Ax = k * ax, Ay = k * ay, Az = k * az;               // dt (A u)_i
         if (RESIDUAL0) {
             float4 r = make_float4(Ax, Ay, Az, ui.w);

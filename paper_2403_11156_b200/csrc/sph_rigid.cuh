@@ -227,7 +227,7 @@ k_rigid_step(SimConst c, SphRigidBody *__restrict__ bodies, float tminx, float t
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        double dt = c.dt, M = B.mass;
+        double dt = step_dt(c), M = B.mass;
         double g[3] = { c.gx, c.gy, c.gz };
         double V[3], w[3], X[3], q[4], R[9];
         for (int a = 0; a < 3; ++a) { V[a] = B.lin_vel[a] + dt * (M * g[a] + sh[a]) / M; w[a] = B.ang_vel[a]; X[a] = B.com[a]; }
@@ -279,8 +279,18 @@ k_rigid_step(SimConst c, SphRigidBody *__restrict__ bodies, float tminx, float t
 enum { LOOP_DIV = 0, LOOP_DENS = 1, LOOP_CG = 2 };
 constexpr int kCtrlThreads = 1024;   // one CTA sums the per-CTA partials: wide, so that the loads overlap
 
-__global__ void k_step_begin(DevStats *st, DevControl *ctl)
+// Start of a step: choose its dt (reading R26: dt = clamp(lambda 2r / max|v|, dt_min, dt_max) with the
+// velocities at the step's start -- st->vmax_bits holds their maximum, left there by the previous step's
+// integration or by k_vmax; cfl2r = lambda 2r, 0 = fixed dt), then reset the per-step statistics.
+__global__ void k_step_begin(DevStats *st, DevControl *ctl, float cfl2r, float dt_min, float dt_max)
 {
+    float dt = dt_max;
+    if (cfl2r > 0.f) {
+        float vmax = __uint_as_float(st->vmax_bits);
+        dt = fminf(dt_max, cfl2r / fmaxf(vmax, 1e-30f));
+        dt = fmaxf(dt, dt_min);
+    }
+    ctl->dt = dt;
     st->it_v = 0; st->it_d = 0; st->cg_iters = 0; st->max_iter_hit = 0;
     st->err_v = 0.f; st->err_rho = 0.f; st->cg_residual = 0.f;
     st->oob = 0; st->nan_count = 0; st->vmax_bits = 0u;
@@ -292,9 +302,10 @@ __global__ void k_list_counters_reset(DevStats *st)
     st->oob = 0;
     st->lc.overflow = 0; st->lc.max_f = 0; st->lc.max_b = 0; st->lc.sum_f = 0ull;
 }
-__global__ void k_step_end(DevStats *st)
+__global__ void k_step_end(DevStats *st, const DevControl *ctl)
 {
     st->steps_done += 1;
+    st->dt_last = ctl->dt; st->sim_time += (double)ctl->dt;
     st->total_it_v += st->it_v; st->total_it_d += st->it_d; st->total_cg += st->cg_iters;
 }
 
@@ -347,6 +358,25 @@ k_cg_ctrl2(const float *__restrict__ prr, int nparts, DevControl *ctl, DevStats 
         if (ctl->forced_cg < 0 && !cont && rr_new > tol2) st->max_iter_hit |= 4;
     }
     set_loop_condition(h, use_handle, ctl, cont);
+}
+
+// max_i |v_i| of the persistent store into st->vmax_bits (same arithmetic as the integration tail): run
+// before a step whose start velocities were not left by a previous step (first step, after sph_write_state)
+__global__ void __launch_bounds__(256)
+k_vmax(const float4 *__restrict__ vel, int n, unsigned *__restrict__ vmax_bits)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float v2 = 0.f;
+    if (i < n) {
+        float4 v = vel[i];
+        v2 = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
+        if (!isfinite(v2)) v2 = 0.f;
+    }
+    v2 = warp_max(v2);
+    if ((threadIdx.x & 31) == 0) {
+        unsigned vb = __float_as_uint(sqrtf(v2));
+        if (vb > *(volatile unsigned *)vmax_bits) atomicMax(vmax_bits, vb);
+    }
 }
 
 }  // namespace sph

@@ -100,9 +100,15 @@ def resync_step(g, o, scene, method="dfsph"):
         st = g.sph_read_stats()
         fcg = st["cg_iters"] if scene.params["viscosity_mode"] == 2 else -1
         fv = st["it_v"] if scene.params["enable_divergence_solve"] else -1
+        if scene.params.get("cfl_factor", 0.0) > 0.0:
+            o.set_forced_dt(st["dt_last"])      # the GPU's fp32 choice of dt (several values are valid, R20 / R26)
         o.step_dfsph(forced_v=fv, forced_d=st["it_d"], forced_cg=fcg)
+        o.set_forced_dt(0.0)
     else:
         g.sph_step_wcsph(1)
         st = g.sph_read_stats()
+        if scene.params.get("cfl_factor", 0.0) > 0.0:
+            o.set_forced_dt(st["dt_last"])
         o.step_wcsph()
+        o.set_forced_dt(0.0)
     return field_errors(g, o, scene), st

@@ -465,3 +465,65 @@ def test_config1_wcsph_and_dfsph_centre_of_mass_agree(B):
     g.close()
     d = 2.0 * sc.params["particle_radius"]
     assert np.linalg.norm(com_d - com_w) <= 0.25 * d, (com_d, com_w)
+
+
+# ------------------------------------------------------------------ CFL-adaptive time step (R26, NEXT-1)
+
+def test_cfl_adaptive_time_step_parity(B, oracle):
+    """cfl_factor > 0: dt is chosen on the device before every step from max |v| at the step's start
+    (after create, after sph_write_state, and from the previous step's integration).  The GPU's dt
+    equals the rule evaluated on the host from the same velocities; whole-step parity with the
+    oracle at that dt; the free-running oracle picks the same dt to fp32 accuracy; graph and
+    host-driven launches agree bit for bit; simulated time is the sum of the steps' dt."""
+    import torch
+    lam, dt_max, dt_min = 0.4, 4e-4, 2e-5
+    sc = scenes.dam_break((14, 14, 14), (28, 16, 20), steps=20, cfl_factor=lam, dt_min=dt_min)
+    two_r = 2.0 * sc.params["particle_radius"]
+
+    def rule(vel):
+        vm = float(torch.linalg.vector_norm(vel.to(torch.float64), dim=1).max())
+        return min(dt_max, max(dt_min, lam * two_r / max(vm, 1e-30)))
+
+    g, o = make_pair(sc, oracle)
+    # v = 0 at the start: dt = dt_max
+    e, st = resync_step(g, o, sc)
+    check_errors(e, sc)
+    assert st["dt_last"] == pytest.approx(dt_max, rel=1e-7)
+    # fast fluid written through the ABI: the rule must see the NEW velocities
+    v = g.sph_read_state(B.VEL).clone()
+    v[:, 0] += 30.0
+    g.sph_write_state(B.VEL, v)
+    expect = rule(g.sph_read_state(B.VEL))
+    e, st = resync_step(g, o, sc)
+    check_errors(e, sc)
+    assert st["dt_last"] == pytest.approx(expect, rel=2e-6) and st["dt_last"] < dt_max
+    # following steps take max |v| from the previous step's integration tail
+    t = st["sim_time"]
+    for k in range(6):
+        expect = rule(g.sph_read_state(B.VEL))
+        e, st = resync_step(g, o, sc)
+        check_errors(e, sc)
+        assert st["dt_last"] == pytest.approx(expect, rel=2e-6), k
+        t += st["dt_last"]
+        assert st["sim_time"] == pytest.approx(t, rel=1e-6)
+        assert st["err_rho"] < 1e-3
+    # free-running oracle from the same state chooses the same dt
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_step_dfsph(1); o.step_dfsph()
+    assert o.stats()["dt_last"] == pytest.approx(g.sph_read_stats()["dt_last"], rel=2e-6)
+    # lower clamp
+    v = g.sph_read_state(B.VEL).clone(); v[:, 1] += 5000.0
+    g.sph_write_state(B.VEL, v)
+    g.sph_step_wcsph(1)
+    assert g.sph_read_stats()["dt_last"] == pytest.approx(dt_min, rel=1e-7)
+    g.close(); o.close()
+    # CUDA-graph and host-driven launches: identical trajectories
+    outs = []
+    for graph in (1, 0):
+        gg = B.Sim.from_scene(sc, use_cuda_graph=graph)
+        v = gg.sph_read_state(B.VEL).clone(); v[:, 0] += 25.0
+        gg.sph_write_state(B.VEL, v)
+        gg.sph_step_dfsph(8)
+        outs.append((gg.sph_read_state(B.POS).clone(), gg.sph_read_stats()["sim_time"]))
+        gg.close()
+    assert torch.equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1]
