@@ -315,7 +315,7 @@ int enqueue_density(SphSim *s, const LoopCtx &lc, bool divp)
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
     LoopHandle lh{ lc.h, lc.use_handle };
-#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->pvB, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl, s->stats, lh)
+#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->pvB, s->bvel_s, s->alpha, s->posk, s->ctl, s->stats, lh)
     if (s->prm.use_neighbor_list) {
         if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
     } else {
@@ -390,7 +390,7 @@ int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, PV *vel, int first)
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
     LoopHandle lh{ lc.h, lc.use_handle };
-#define SOLP(MODE, DYN) LAUNCH(s, (k_solver_p<LIST, MODE, DYN>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->partial, s->ctl, s->stats, lh, first)
+#define SOLP(MODE, DYN) LAUNCH(s, (k_solver_p<LIST, MODE, DYN>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->ctl, s->stats, lh, first)
     if (mode == MODE_DIV) { if (dyn) SOLP(MODE_DIV, true); else SOLP(MODE_DIV, false); }
     else                  { if (dyn) SOLP(MODE_DENS, true); else SOLP(MODE_DENS, false); }
 #undef SOLP

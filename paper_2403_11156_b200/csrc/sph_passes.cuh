@@ -13,9 +13,9 @@
 //   posk[nf] float4  x, y, z, kappa_i/rho_i (written by every P-pass, gathered by the C-pass:
 //                                            one 16-byte gather per neighbour instead of two)
 //   bpos[nb] float4  x, y, z, Psi           bvel[nb] float4 vx, vy, vz, -
-// Neighbour lists (built once per step by k_density_alpha, consumed by every later pass):
-//   warp tile w = i / 32 owns rows [w*K*32, (w+1)*K*32); entry k of particle i is at
-//   tile + k*32 + (i & 31), so that a warp reads row k with one coalesced 128-byte load.
+// Neighbour lists (built once per step by k_build_lists, consumed by every later pass): warp-tiled,
+//   16-bit (x-run, offset) entries for fluid neighbours, 32-bit indices for boundary neighbours; see
+//   list_tile() and for_each_neighbor() below.
 #pragma once
 #include "sph_common.cuh"
 
@@ -25,7 +25,6 @@ enum { MODE_DIV = 0, MODE_DENS = 1 };
 
 struct __align__(32) PV { float4 x, v; };   // position (x, y, z, -) | velocity (vx, vy, vz, rho)
 
-// 32 bytes (aligned) through the read-only path with one instruction
 // list words are read once per pass: keep them out of L1, which the gathers need
 __device__ __forceinline__ uint32_t ldg_stream(const uint32_t *p)
 {
@@ -40,6 +39,7 @@ __device__ __forceinline__ void ldg256_if(bool on, const float4 *p, float4 &a, f
         : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w)
         : "l"(p), "r"((unsigned)on));
 }
+// 32 bytes (aligned) through the read-only path with one instruction
 __device__ __forceinline__ void ldg256(const float4 *p, float4 &a, float4 &b)
 {
     asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
@@ -508,11 +508,11 @@ __device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevCo
 // neighbour loop (A5): D_i needs only the velocities of the step's start, and kappa^v_i the
 // alpha_i that this very loop produces -- one full neighbour pass less per step.  It writes
 // posk[i] = (x_i, kappa^v_i / rho_i) (0 when the divergence solve is switched off) and the CTA
-// partial of R_i = max(D_i, 0).
+// error sum of R_i = max(D_i, 0) (solver_tail).
 template <bool LIST, bool DIVP, bool DYN>
 __global__ void __launch_bounds__(kBlock)
 k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
-                float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
+                float *__restrict__ alpha, float4 *__restrict__ posk,
                 DevControl *ctl, DevStats *st, LoopHandle lh)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
@@ -581,12 +581,12 @@ k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
 // DIV  (Eq. 10 source; R15): R_i = max(D_i, 0), kappa^v_i = alpha_i R_i / dt, term = R_i
 // DENS (Eq. 8-9; R15) : E_i = max(rho_i + dt D_i, rho0) - rho0,
 //                                          kappa_i = alpha_i E_i / dt^2, term = E_i
-// Writes posk[i] = (x_i, kappa_i / rho_i) and one partial sum of `term` per CTA.
+// Writes posk[i] = (x_i, kappa_i / rho_i); the error term is reduced by solver_tail (A12).
 
 template <bool LIST, int MODE, bool DYN>
 __global__ void __launch_bounds__(kBlock)
 k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel,
-           const float *__restrict__ alpha, float4 *__restrict__ posk, float *__restrict__ partial,
+           const float *__restrict__ alpha, float4 *__restrict__ posk,
            DevControl *ctl, DevStats *st, LoopHandle lh, int first)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
