@@ -22,7 +22,10 @@
  * antisymmetry; brute-force neighbour sets; lattice rest density and alpha; two-particle
  * closed form; planar Akinci volumes; free fall; momentum invariants of both solvers;
  * fluid + rigid momentum exchange (Eq. 14); implicit-viscosity operator symmetry and CG
- * vs dense solve; explicit Laplacian of a quadratic field; rigid stand-in closed forms.
+ * vs dense solve; explicit Laplacian of a quadratic field; rigid stand-in closed forms;
+ * scale of the implicit-viscosity operator (tied to the Eq. 15 lattice constant); boundary
+ * terms of D and U against a moving one-sample body (closed form, incl. the Eq. 14 reaction);
+ * torque / angular response through total angular momentum of fluid + body.
  * Multi-step GPU-vs-oracle trajectories beyond a few steps: "parity unpinned" (chaotic),
  * only statistics are compared.
  */

@@ -620,6 +620,8 @@ def test_golden_closed_forms_are_what_the_formulas_give():
     definition (no oracle involved), so a typo in the fixture cannot silently weaken a pin."""
     g = _golden()
     assert g["kernel_sigma_h3"] == pytest.approx(8.0 / np.pi, rel=1e-15)
+    assert g["psi_single_sample_over_rho0_h3"] == pytest.approx(np.pi / 8.0, rel=1e-15)
+    assert g["gradw_at_half_h_times_h4"] == pytest.approx(12.0 / np.pi, rel=1e-15)
     a = 1 - 1 / np.sqrt(2); b = 1 - np.sqrt(3) / 2
     assert g["akinci_volume_one_layer"] == pytest.approx(np.pi / (2 + 8 * a ** 3), abs=1e-6)
     assert g["akinci_volume_two_layers"] == pytest.approx(np.pi / (2.25 + 16 * a ** 3 + 8 * b ** 3), abs=1e-6)
@@ -729,3 +731,163 @@ def test_cfl_time_step_rule_and_free_fall_recurrence(oracle):
                      domain_min=(-1.0, -1.0, 0.0), domain_max=(2.0, 1.0, 6.0))
     fixed.step_dfsph()
     assert fixed.stats()["dt_last"] == 4e-4
+
+
+# ---------------------------------------------------------------- round-2 pins: operator scale, boundary terms, torque
+
+@pytest.mark.parametrize("ratio,expect", [(2, 1.396226), (4, 1.91156)])
+def test_implicit_viscosity_operator_scale(oracle, ratio, expect):
+    """SCALE of Eq. 19 (R4, R21), tied to the pinned Eq. 15: on an interior
+    simple-cubic lattice (rho_i = rho_j = rho_c, m = rho0 s^3) with u = (y^2, 0, 0)
+        (A u)_c = 2(d+2) mu m / rho_c^2 sum_j (...) = nu L (rho0 / rho_c)^2,
+    L = the discrete Laplacian constant of test_explicit_laplacian_of_quadratic_field (1.396226 at
+    h = 2s, 1.91156 at h = 4s; tests/golden/closed_forms.txt), rho_c the oracle's own lattice density.
+    Catches what the symmetry / null-space / CG-vs-dense pins cannot: a wrong 2(d+2) (8 for 10), mu m /
+    (rho_i rho_j) off by a constant (rho0 missing in mu = nu rho0, m^2 for m, rho_i^2 only)."""
+    sp = H / ratio
+    n = 4 * ratio + 1                 # centre +- 2h: the centre's neighbours are interior particles too
+    pos = _lattice(n, sp)
+    nu = 3.0
+    sim = make_sim(oracle, np.zeros((len(pos), 3), np.float32), particle_mass=RHO0 * sp ** 3,
+                   kinematic_viscosity=nu, viscosity_mode=2,
+                   domain_min=(-H, -H, -H), domain_max=tuple([n * sp + H] * 3))
+    sim.set_state(pos, np.zeros_like(pos))
+    sim.build_grid(); sim.compute_density_alpha()
+    c = (n // 2) * (n * n + n + 1)
+    rho = sim.density()
+    st, idx = sim.neighbors(0)
+    nb = idx[st[c]:st[c + 1]]
+    assert len(nb) > 20 and np.abs(rho[nb] - rho[c]).max() < 1e-9 * rho[c]      # interior: one density
+    assert abs(rho[c] / RHO0 - 1) < 0.01 and rho[c] != RHO0
+    u = np.zeros_like(pos); u[:, 0] = pos[:, 1] ** 2
+    Au = sim.viscosity_operator(u)
+    want = nu * expect * (RHO0 / rho[c]) ** 2
+    assert Au[c, 0] == pytest.approx(want, rel=2e-5)
+    assert abs(Au[c, 1]) < 1e-9 * want and abs(Au[c, 2]) < 1e-9 * want
+    # and it is the explicit formula with rho_j = rho_c, up to the extra rho0 / rho_c of mu m/(rho_i rho_j)
+    acc = sim.explicit_viscosity_accel(u, np.full(len(pos), rho[c]))
+    assert Au[c, 0] == pytest.approx(acc[c, 0] * RHO0 / rho[c], rel=1e-12)
+
+
+def _one_fluid_one_dynamic_sample(oracle, vi, vk, **prm):
+    """fluid particle i at the origin-ish point, ONE boundary sample k = a dynamic single-sample body at
+    distance h/2 in +x, moving with v_k (its sample velocity is lin_vel: no rotation arm)."""
+    xi = np.array([0.1, 0.1, 0.1]); xk = xi + np.array([0.5 * H, 0.0, 0.0])
+    body = scenes.Body(0, 1, dynamic=1, mass=0.5, inertia_body=(1e-3, 1e-3, 1e-3), com=tuple(xk),
+                       lin_vel=tuple(vk), contact_radius=0.0)
+    far = 50.0
+    sim = make_sim(oracle, xi[None, :], fvel=np.asarray(vi, dtype=np.float64)[None, :], bpos=xk[None, :],
+                   bodies=[body], gravity=(0.0, 0.0, 0.0), tank_min=(-far,) * 3, tank_max=(far,) * 3, **prm)
+    return sim, xi, xk
+
+
+def test_boundary_terms_of_density_rate_and_pressure_update(oracle):
+    """Boundary sums of D_i and U_i with a MOVING sample (Eq. 6 / 10 / 13 / 14, PAPER.md:110, 156, 200, 204;
+    R8): one fluid particle at h/2 from a one-sample dynamic body.  By hand: Psi = rho0 / W(0) (Eq. 11),
+    gradW_ik = -(1.5 sigma / h) n with n = (x_i - x_k)/|.| = -e_x, so
+        D = Psi (v_i - v_k).gradW_ik,   err_v = dt D / rho0,
+    and one forced divergence iteration (alpha = rho / |Psi gradW|^2, T = 0) removes exactly the approaching
+    normal relative velocity, v_i' = v_i - ((v_i - v_k).n) n, with the Eq. 14 reaction F_k = -m (v_i' - v_i)/dt.
+    A separating pair is untouched (R15).  Catches: v_k dropped or with the wrong sign in D, m in place of
+    Psi_k, Psi_k^2, a wrong sign or missing m in the reaction."""
+    dt = 4e-4
+    gold = _golden()
+    psi = gold["psi_single_sample_over_rho0_h3"] * RHO0 * H ** 3      # = rho0 / W(0)
+    g = gold["gradw_at_half_h_times_h4"] / H ** 4                     # = 1.5 sigma / h
+    assert psi == pytest.approx(RHO0 / SIGMA, rel=1e-14) and g == pytest.approx(1.5 * SIGMA / H, rel=1e-14)
+    m = RHO0 * S ** 3
+    vi = np.array([0.05, 0.2, -0.1]); vk = np.array([-0.35, 0.1, 0.3])
+    sim, xi, xk = _one_fluid_one_dynamic_sample(oracle, vi, vk, dt=dt)
+    assert sim.psi()[0] == pytest.approx(psi, rel=1e-12)
+    assert np.allclose(sim.boundary_vel()[0], vk, atol=1e-7)
+    sim.build_grid(); sim.compute_density_alpha()
+    v1, it = sim.divergence_solve(vi[None, :], forced=1)
+    n = np.array([-1.0, 0.0, 0.0])
+    D = psi * np.dot(vi - vk, -g * n)                 # = psi * 0.4 * g > 0: approaching
+    assert D > 0
+    assert sim.stats()["err_v"] == pytest.approx(dt / RHO0 * D, rel=1e-6)
+    want = vi - np.dot(vi - vk, n) * n
+    assert np.allclose(v1[0], want, rtol=1e-6, atol=1e-9)
+    assert abs(v1[0, 0] - vk[0]) < 1e-6               # normal velocities now equal
+    F = sim.boundary_force()[0]
+    assert np.allclose(F, -m * (v1[0] - vi) / dt, rtol=1e-6, atol=1e-9 * m / dt)
+    assert F[0] > 0                                   # the fluid pushes the sample away from itself (+x)
+    # v_k matters: the same fluid velocity against a sample at rest approaches 8x slower
+    sim0, _, _ = _one_fluid_one_dynamic_sample(oracle, vi, np.zeros(3), dt=dt)
+    sim0.build_grid(); sim0.compute_density_alpha()
+    sim0.divergence_solve(vi[None, :], forced=1)
+    assert sim0.stats()["err_v"] == pytest.approx(dt / RHO0 * psi * g * vi[0], rel=1e-6)
+    # separating pair: D < 0 is clamped (R15), nothing moves, no reaction
+    sims, _, _ = _one_fluid_one_dynamic_sample(oracle, vk, vi, dt=dt)
+    sims.build_grid(); sims.compute_density_alpha()
+    v2, _ = sims.divergence_solve(vk[None, :], forced=1)
+    assert np.array_equal(v2[0], vk)
+    assert np.all(sims.boundary_force()[0] == 0.0)
+    # the density solve sees the same boundary term: rho* = rho + dt D, kappa = alpha (rho* - rho0)/dt^2
+    simd, _, _ = _one_fluid_one_dynamic_sample(oracle, vi, vk, dt=dt, particle_mass=3.0 * m)
+    simd.build_grid(); simd.compute_density_alpha()
+    rho = 3.0 * m * SIGMA + psi * SIGMA / 4
+    assert simd.density()[0] == pytest.approx(rho, rel=1e-6) and rho > RHO0
+    v3, _ = simd.density_solve(vi[None, :], forced=1)
+    E = rho + dt * D - RHO0
+    assert simd.stats()["err_rho"] == pytest.approx(E / RHO0, rel=1e-6)
+    # v' = v - dt Psi (kappa/rho) gradW = v + (E / (dt Psi g)) n
+    assert np.allclose(v3[0], vi + E / (dt * psi * g) * n, rtol=1e-6, atol=1e-9)
+
+
+def _angular_momentum_about_origin(sim, m):
+    """sum x cross m v (fluid) + X cross M V + R I_b R^T omega (body 0), fp64."""
+    b = sim.bodies()[0]
+    w, x, y, z = b["quat"]
+    Rm = np.array([[1 - 2 * (y * y + z * z), 2 * (x * y - w * z), 2 * (x * z + w * y)],
+                   [2 * (x * y + w * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w * x)],
+                   [2 * (x * z - w * y), 2 * (y * z + w * x), 1 - 2 * (x * x + y * y)]])
+    spin = Rm @ (b["inertia_body"] * (Rm.T @ b["ang_vel"]))
+    orbital = np.cross(b["com"], b["mass"] * b["lin_vel"])
+    fluid = m * np.cross(sim.pos(), sim.vel()).sum(0)
+    return fluid + orbital + spin, spin, b
+
+
+def test_torque_conserves_total_angular_momentum(oracle):
+    """tau = sum_k (x_k - X) x F_k and the angular response of the rigid stand-in (Eq. 14, PAPER.md:204;
+    R18): g = 0, a box with a small fluid block pressed against an OFF-CENTRE part of its top face.  Pair
+    forces are central (along x_i - x_k), so the total angular momentum about a fixed point,
+        sum_i x_i x m v_i + X x M V + I_w omega,
+    is conserved by every C-pass exactly and by the explicit body integration to O(dt^2 omega^2); it must
+    stay constant to a small fraction of the spin the body picks up.  A flipped cross product (F x r), a
+    torque about the origin instead of X, a missing I^-1 or a transposed R fail it (error ~ 2x the spin);
+    the linear-momentum pin cannot see any of them."""
+    dt = 4e-4
+    sc = scenes.free_block((3, 3, 2), jitter=0.0, vel_scale=0.0, seed=0)
+    pos = sc.fluid_pos.astype(np.float64)
+    pos += np.array([0.5, 0.5, 0.5]) - pos.min(0)
+    vel = np.zeros_like(pos); vel[:, 2] = -1.0
+    size = (0.16, 0.1, 0.06)
+    # box top face 0.9 s below the lowest fluid layer; fluid over the +x end of the face, off-centre in y too
+    ctr = (pos[:, 0].mean() - 0.05, pos[:, 1].mean() - 0.02, pos[:, 2].min() - 0.9 * S - 0.5 * size[2])
+    pts, body = scenes.make_rigid_box(ctr, size, 600.0, S)
+    body.first_particle = 0; body.n_particles = len(pts)
+    far = 50.0
+    sim = make_sim(oracle, pos.astype(np.float32), fvel=vel, bpos=pts, bodies=[body], gravity=(0.0, 0.0, 0.0),
+                   dt=dt, tank_min=(-far,) * 3, tank_max=(far,) * 3)
+    m = sim.mass()
+    L0, spin0, _ = _angular_momentum_about_origin(sim, m)
+    assert np.all(spin0 == 0)
+    Ls = []
+    for _ in range(3):
+        sim.step_dfsph()
+        Ls.append(_angular_momentum_about_origin(sim, m))
+    L3, spin3, b = Ls[-1]
+    I = np.asarray(b["inertia_body"])
+    assert np.linalg.norm(b["ang_vel"]) > 1e-3                   # the body was set spinning ...
+    assert abs(b["ang_vel"][1]) > 10 * abs(b["ang_vel"][2])      # ... mainly about y (fluid over the +x end)
+    assert b["ang_vel"][1] > 0                                   # -z force at +x arm: tau_y = r_z F_x - r_x F_z > 0
+    assert b["lin_vel"][2] < -1e-4                               # and pushed down
+    # integrator error of the explicit body update: I_w is taken at the old orientation, so each step leaves
+    # dt |omega x I_w omega| + O(dt^2) unaccounted; everything else is exact
+    bound = 3 * 2.0 * dt * np.linalg.norm(np.cross(b["ang_vel"], spin3)) + 1e-9 * np.linalg.norm(spin3)
+    assert bound < 2e-2 * np.linalg.norm(spin3)      # a flipped or mis-centred torque is off by ~2 |spin|
+    for L, _, _ in Ls:
+        assert np.abs(L - L0).max() < bound, (L - L0, spin3, bound)
+    # magnitude of the response: omega = I_w^-1 L_spin with the body still (almost) axis-aligned
+    assert np.allclose(b["ang_vel"][:2], (spin3 / I)[:2], rtol=2e-2)
