@@ -15,7 +15,9 @@
  *     only to capture CUDA-graph loop bodies, never to run work) and a few KB of pinned host
  *     memory.
  *   - all work is enqueued asynchronously on the cudaStream_t given to sph_create(); the only
- *     calls that synchronise that stream are sph_read_stats(), host-buffer copies of
+ *     calls that synchronise that stream are sph_read_stats(), sph_launch_count(),
+ *     sph_read_kernel_times(), sph_set_forced_iterations() (its three words travel through a
+ *     pinned block that the next call reuses), host-buffer copies of
  *     sph_read_state()/sph_write_state(), sph_create() itself (it computes the Akinci
  *     volumes) and the step calls when SphParams.use_cuda_graph == 0 (debug mode: the
  *     solver loops are then driven from the host).
@@ -60,7 +62,8 @@ typedef struct SphParams {
     float domain_max[3];       /*   the edge cells and counted in SphStats.oob_count (R11)   */
     float tank_min[3];         /* AABB used only by the rigid-body wall-contact stand-in (R18) */
     float tank_max[3];
-    int   viscosity_mode;      /* 0 none, 1 explicit Eq. 15, 2 implicit Eq. 16-19 (CG) */
+    int   viscosity_mode;      /* 0 none, 1 explicit Eq. 15, 2 implicit Eq. 16-19 (CG; DFSPH steps only:
+                                  sph_step_wcsph returns SPH_ESTATE); anything else: SPH_EINVAL at create */
     float kinematic_viscosity; /* nu = mu / rho0 */
     float cg_rel_tol;          /* |r|_2 <= tol |b|_2                  reading R23 */
     int   cg_max_iter;
@@ -188,14 +191,24 @@ int sph_step_dfsph(SphSim *sim, int n_steps);
 int sph_step_wcsph(SphSim *sim, int n_steps);
 
 /* Override the iteration counts of the next steps: -1 = tolerances decide, >= 0 = exactly that
- * many iterations of the divergence solve / density solve / CG.  Takes effect without re-capture. */
+ * many iterations of the divergence solve / density solve / CG.  Takes effect without re-capture.
+ * Synchronises the stream. */
 int sph_set_forced_iterations(SphSim *sim, int forced_v, int forced_d, int forced_cg);
 
 /* Copy one field out (un-permuted to original id order) / in.  `bytes` must equal the field's
  * size.  is_host = 0: dst/src is a device pointer, copy is asynchronous on the stream;
  * is_host = 1: host pointer, the call returns after the copy has completed.
  * sph_write_state (any writable field) invalidates grid-derived fields until the next
- * sph_build_grid / step. */
+ * sph_build_grid / step.  Boundary fields take effect at that next sph_build_grid / step call:
+ *   SPH_FIELD_BOUNDARY_POS : the samples' world positions are replaced; their body-frame coordinates
+ *                            (pose of their body as it is then) and the Akinci volumes Psi_k (Eq. 11,
+ *                            PAPER.md:178) are recomputed; the sorted boundary store is rebuilt;
+ *   SPH_FIELD_BOUNDARY_VEL : the samples' velocities are replaced (for a dynamic body until its next
+ *                            rigid step derives them from the body state again);
+ *   SPH_FIELD_RIGID_BODIES : the body states are replaced and the samples of DYNAMIC bodies re-posed,
+ *                            x_k = X + R(q) xbar_k, v_k = V + omega x (x_k - X) -- except for what a
+ *                            write of BOUNDARY_POS / BOUNDARY_VEL since the last refresh set directly.
+ *                            first_particle / n_particles / dynamic must not change. */
 int sph_read_state(SphSim *sim, int field, void *dst, size_t bytes, int is_host);
 int sph_write_state(SphSim *sim, int field, const void *src, size_t bytes, int is_host);
 

@@ -55,7 +55,7 @@ struct SphSim {
     float4 *posA = nullptr, *velA = nullptr, *posB = nullptr, *posk = nullptr;
     PV *pvB = nullptr, *pvC = nullptr;   // { pos | vel, rho } records of the passes; pvC: output of explicit viscosity
     int *idA = nullptr, *idB = nullptr;
-    float *alpha = nullptr;
+    float *alpha = nullptr, *rho = nullptr;
     GridBufs gf, gb;
     uint16_t *nl_f = nullptr;       // 16-bit (run, offset) entries, warp-tiled (sph_passes.cuh)
     int *nl_b = nullptr, *ncount = nullptr;
@@ -73,6 +73,7 @@ struct SphSim {
     size_t staging_bytes = 0;
     // host
     int *pinned = nullptr;          // small pinned block (loop predicate, stats)
+    int boundary_dirty = 0;         // DIRTY_* bits: boundary fields written through sph_write_state since the last refresh
     bool vmax_valid = false;        // stats->vmax_bits = max |v| of the persistent store (needed by the CFL rule)
     bool derived_valid = false;     // B-order fields (rho, alpha, lists, cell_start) match the store
     cudaGraphExec_t exec[2] = { nullptr, nullptr };   // 0 DFSPH, 1 WCSPH
@@ -126,6 +127,21 @@ inline cudaEvent_t take_event(SphSim *s)
     return e;
 }
 
+// host (pageable) -> device through pinned memory, ordered on the simulation's stream; returns after the copy
+// has completed (the stream given to sph_create may be non-blocking: nothing may go through the legacy stream)
+int upload(SphSim *s, void *dst_dev, const void *src_host, size_t bytes)
+{
+    if (bytes == 0) return SPH_OK;
+    void *tmp = nullptr;
+    CUDA_TRY(s, cudaMallocHost(&tmp, bytes));
+    memcpy(tmp, src_host, bytes);
+    cudaError_t e = cudaMemcpyAsync(dst_dev, tmp, bytes, cudaMemcpyHostToDevice, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    cudaFreeHost(tmp);
+    CUDA_TRY(s, e);
+    return SPH_OK;
+}
+
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
 
 struct DeviceGuard {
@@ -160,6 +176,8 @@ bool make_geom(const SphParams &p, Geom &g, std::string &why)
     return true;
 }
 
+enum { DIRTY_BPOS = 1, DIRTY_BVEL = 2, DIRTY_BODIES = 4 };
+
 int list_cap(int v, int vmax) { if (v <= 0) v = 64; v = (v + 3) & ~3; if (v > vmax) v = vmax; return v; }
 
 bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &why)
@@ -171,6 +189,7 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     if (!(p.cfl_factor >= 0.f) || !(p.dt_min >= 0.f) || p.dt_min > p.dt) {
         why = "cfl_factor must be >= 0 and 0 <= dt_min <= dt"; return false;
     }
+    if (p.viscosity_mode < 0 || p.viscosity_mode > 2) { why = "viscosity_mode must be 0 (none), 1 (explicit, Eq. 15) or 2 (implicit, Eq. 16-19)"; return false; }
     if (!make_geom(p, c.g, why)) return false;
     c.nf = nf; c.nb = nb;
     c.kf = list_cap(p.max_fluid_neighbors, kMaxListCap);
@@ -211,6 +230,7 @@ size_t layout(SphSim &s, void *base)
     s.pvC = s.prm.viscosity_mode == 1 ? w.take<PV>(nf1) : nullptr;
     s.posk = w.take<float4>(nf1);
     s.alpha = w.take<float>(nf1);
+    s.rho = w.take<float>(nf1);
     s.gf.n = (int)nf;
     s.gf.key = w.take<int>(nf1); s.gf.off = w.take<int>(nf1); s.gf.slot = w.take<int>(nf1);
     s.gf.cell_start = w.take<int>(s.cs_len);
@@ -279,6 +299,33 @@ int enqueue_boundary_grid(SphSim *s, cudaStream_t st)
     return enqueue_grid(s, st, s->gb, s->borig_pos, s->borig_vel, nullptr, s->bpos_s, s->bvel_s, s->bid_s, nullptr, false);
 }
 
+// Boundary fields written through sph_write_state take effect here (start of sph_build_grid / of a step call):
+//  * body states written: the samples of dynamic bodies are re-posed from them (unless sample positions /
+//    velocities were written as well: those win);
+//  * sample positions written: body-frame coordinates and the Akinci volumes Psi (Eq. 11) are recomputed;
+//  * in every case the sorted boundary store that the passes read is rebuilt.
+int refresh_boundary(SphSim *s)
+{
+    const int dirty = s->boundary_dirty;
+    if (!dirty) return SPH_OK;
+    s->boundary_dirty = 0;
+    const int nb = s->c.nb;
+    if (nb <= 0) return SPH_OK;
+    cudaStream_t st = s->stream;
+    if (dirty & DIRTY_BODIES) {
+        const int set_pos = !(dirty & DIRTY_BPOS), set_vel = !(dirty & DIRTY_BVEL);
+        if (set_pos || set_vel)
+            LAUNCH(s, k_body_pose, cdiv(nb, 256), 256, st, s->brest, s->bbody, s->bodies, nb, s->borig_pos, s->borig_vel, set_pos, set_vel);
+    }
+    if (dirty & DIRTY_BPOS)
+        LAUNCH(s, k_body_rest, cdiv(nb, 256), 256, st, s->borig_pos, s->bbody, s->bodies, nb, s->brest, s->borig_vel, 0);
+    int rc = enqueue_boundary_grid(s, st);
+    if (rc) return rc;
+    if (dirty & DIRTY_BPOS)
+        LAUNCH(s, k_boundary_psi, cdiv(nb, kBlock), kBlock, st, s->c, s->bpos_s, s->bid_s, s->gb.cell_start, s->bbody, s->borig_pos);
+    return SPH_OK;
+}
+
 // Solver loops.  graph mode: a conditional WHILE node whose body is captured on the helper
 // stream; host mode: the host reads the predicate after every iteration.
 struct LoopCtx {
@@ -315,7 +362,7 @@ int enqueue_density(SphSim *s, const LoopCtx &lc, bool divp)
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
     LoopHandle lh{ lc.h, lc.use_handle };
-#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->pvB, s->bvel_s, s->alpha, s->posk, s->ctl, s->stats, lh)
+#define DENS(LIST, DIVP, DYN) LAUNCH(s, (k_density_alpha<LIST, DIVP, DYN>), s->nblocks, kBlock, lc.st, p, s->pvB, s->bvel_s, s->alpha, s->rho, s->posk, s->ctl, s->stats, lh)
     if (s->prm.use_neighbor_list) {
         if (!divp) DENS(true, false, false); else if (dyn) DENS(true, true, true); else DENS(true, true, false);
     } else {
@@ -405,6 +452,7 @@ int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, PV *vel)
     const bool dyn = s->c.has_dynamic != 0;
     CTail t;
     t.ctl = s->ctl;
+    t.rho = s->rho;
     t.add_gravity = s->prm.viscosity_mode != 1;
     t.id = s->idB; t.pos_out = s->posA; t.vel_out = s->velA; t.id_out = s->idA;
     t.vmax_bits = &s->stats->vmax_bits; t.nan_count = &s->stats->nan_count;
@@ -487,7 +535,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
             LoopCtx plain{ st, 0, 0 };
             rc = enqueue_density(s, plain, false);
             if (rc) return rc;
-            LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->pvB, s->posk);
+            LAUNCH(s, k_wcsph_eos, cdiv(nf, 256), 256, st, s->c, s->posB, s->rho, s->pvB, s->posk);
             if (s->prm.viscosity_mode == 1) {
                 LAUNCH(s, (k_explicit_viscosity<LIST, true>), s->nblocks, kBlock, st, p, s->pvB, s->pvC);
                 vcur = s->pvC;
@@ -536,7 +584,9 @@ int do_steps(SphSim *s, int method, int n_steps)
 {
     if (!s) return SPH_EINVAL;
     if (n_steps < 0) { s->err = "n_steps < 0"; return SPH_EINVAL; }
+    if (method == 1 && s->prm.viscosity_mode == 2) { s->err = "sph_step_wcsph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
     DeviceGuard dg(s->device);
+    if (n_steps > 0) { int rc = refresh_boundary(s); if (rc) return rc; }
     if (s->prm.cfl_factor > 0.f && !s->vmax_valid && n_steps > 0 && s->c.nf > 0) {
         // the CFL rule needs max |v| at the start of the step; later steps get it from the integration tail
         CUDA_TRY(s, cudaMemsetAsync(&s->stats->vmax_bits, 0, sizeof(unsigned), s->stream));
@@ -592,7 +642,7 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
     switch (field) {
     case SPH_FIELD_POS: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->posA, s->idA, nf, (float *)out); break;
     case SPH_FIELD_VEL: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->velA, s->idA, nf, (float *)out); break;
-    case SPH_FIELD_DENSITY: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, &s->pvB->v, s->idB, nf, (float *)out, 2); break;
+    case SPH_FIELD_DENSITY: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->rho, s->idB, nf, (float *)out); break;
     case SPH_FIELD_ALPHA: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->alpha, s->idB, nf, (float *)out); break;
     case SPH_FIELD_KAPPA_OVER_RHO: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posk, s->idB, nf, (float *)out, 1); break;
     case SPH_FIELD_CELL_START:
@@ -629,10 +679,10 @@ int import_field(SphSim *s, int field, const void *src, size_t bytes)
     switch (field) {
     case SPH_FIELD_POS: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->posA); break;
     case SPH_FIELD_VEL: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->velA); s->vmax_valid = false; break;
-    case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_pos); break;
-    case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_vel); break;
+    case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_pos); s->boundary_dirty |= DIRTY_BPOS; break;
+    case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_vel); s->boundary_dirty |= DIRTY_BVEL; break;
     case SPH_FIELD_RIGID_BODIES:
-        CUDA_TRY(s, cudaMemcpyAsync(s->bodies, src, bytes, cudaMemcpyDeviceToDevice, st)); break;
+        CUDA_TRY(s, cudaMemcpyAsync(s->bodies, src, bytes, cudaMemcpyDeviceToDevice, st)); s->boundary_dirty |= DIRTY_BODIES; break;
     default: s->err = "field is not writable"; return SPH_EINVAL;
     }
     return SPH_OK;
@@ -723,7 +773,6 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
             CARVE((k_cg_apply<true, true>)); CARVE((k_cg_apply<true, false>));
 #undef CARVE
         }
-        if (getenv("SPH_BCARVE")) CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributePreferredSharedMemoryCarveout, atoi(getenv("SPH_BCARVE"))));
         CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (kMaxListCap + kStageExtra) * 64 * (kBlock / 32)));
         const int nf = s->c.nf, nb = s->c.nb;
@@ -751,21 +800,16 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
         // boundary store
         if (s->nbodies > 0) {
             CUDA_TRY(s, cudaStreamSynchronize(st));       // pinned block is reused below
-            if (sizeof(SphRigidBody) * (size_t)s->nbodies <= 4096) {
-                memcpy(s->pinned, bodies, sizeof(SphRigidBody) * (size_t)s->nbodies);
-                CUDA_TRY(s, cudaMemcpyAsync(s->bodies, s->pinned, sizeof(SphRigidBody) * (size_t)s->nbodies, cudaMemcpyHostToDevice, st));
-                CUDA_TRY(s, cudaStreamSynchronize(st));
-            } else {
-                CUDA_TRY(s, cudaMemcpy(s->bodies, bodies, sizeof(SphRigidBody) * (size_t)s->nbodies, cudaMemcpyHostToDevice));
-            }
+            int rc = upload(s, s->bodies, bodies, sizeof(SphRigidBody) * (size_t)s->nbodies);
+            if (rc) return rc;
         }
         CUDA_TRY(s, cudaMemsetAsync(s->gb.cell_start, 0, s->cs_len * sizeof(int), st));
         if (nb > 0) {
             LAUNCH(s, k_pack_vec3, cdiv(nb, 256), 256, st, buf->boundary_pos, nb, s->borig_pos, 0.f);
             CUDA_TRY(s, cudaMemcpyAsync(s->bbody, buf->boundary_body, sizeof(int) * (size_t)nb, cudaMemcpyDeviceToDevice, st));
             CUDA_TRY(s, cudaMemsetAsync(s->bforce, 0, sizeof(float4) * (size_t)nb, st));
-            if (s->ndyn > 0) CUDA_TRY(s, cudaMemcpy(s->dyn_idx, dyn.data(), sizeof(int) * dyn.size(), cudaMemcpyHostToDevice));
-            LAUNCH(s, k_body_rest, cdiv(nb, 256), 256, st, s->borig_pos, s->bbody, s->bodies, nb, s->brest, s->borig_vel);
+            if (s->ndyn > 0) { int rc = upload(s, s->dyn_idx, dyn.data(), sizeof(int) * dyn.size()); if (rc) return rc; }
+            LAUNCH(s, k_body_rest, cdiv(nb, 256), 256, st, s->borig_pos, s->bbody, s->bodies, nb, s->brest, s->borig_vel, 1);
             int rc = enqueue_boundary_grid(s, st);
             if (rc) return rc;
             LAUNCH(s, k_boundary_psi, cdiv(nb, kBlock), kBlock, st, s->c, s->bpos_s, s->bid_s, s->gb.cell_start, s->bbody, s->borig_pos);
@@ -788,6 +832,7 @@ int sph_build_grid(SphSim *s)
     if (!s) return SPH_EINVAL;
     DeviceGuard dg(s->device);
     cudaStream_t st = s->stream;
+    { int rc = refresh_boundary(s); if (rc) return rc; }
     LAUNCH(s, k_list_counters_reset, 1, 1, st, s->stats);
     if (s->c.has_dynamic) {
         int rc = enqueue_boundary_grid(s, st);

@@ -8,7 +8,8 @@
 //                    viscosity) fetch both with ONE 256-bit gather (LDG.E.256, sm_100) -- the list
 //                    passes are bound by L1 gather wavefronts, and one 32-byte sector per neighbour
 //                    costs fewer of them than two 16-byte gathers from two arrays.  rho_i rides in
-//                    v.w: the viscosity sums need rho_j.  pos stays as a packed copy: the list
+//                    v.w (the viscosity sums need rho_j): k_density_alpha writes rho to its own array,
+//                    the first C-pass (or k_wcsph_eos) copies it into the record it rewrites anyway.  pos stays as a packed copy: the list
 //                    builder reads TWO candidates per 256-bit load from it.
 //   posk[nf] float4  x, y, z, kappa_i/rho_i (written by every P-pass, gathered by the C-pass:
 //                                            one 16-byte gather per neighbour instead of two)
@@ -121,12 +122,8 @@ __device__ __forceinline__ void fill_run_table(const Geom &g, const int *__restr
     }
 }
 
-#ifndef SPH_PAIRS1
-#define SPH_PAIRS1 4      // entry pairs per software-pipeline stage when one array is gathered
-#endif
-#ifndef SPH_PAIRS2
-#define SPH_PAIRS2 2      // ... when two arrays are gathered
-#endif
+constexpr int kPairs1 = 4;    // entry pairs per software-pipeline stage when one array is gathered
+constexpr int kPairs2 = 2;    // ... when two arrays (or 32-byte records) are gathered
 
 // Visit every neighbour of fluid particle i (sorted index), fluid first then boundary, both in
 // ascending sorted index:
@@ -151,7 +148,7 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
 {
     const CellOf cell = cell_of(p.c.g, xi, yi, zi);
     if (LIST) {
-        constexpr int PB = NSRC >= 2 ? SPH_PAIRS2 : SPH_PAIRS1;
+        constexpr int PB = NSRC >= 2 ? kPairs2 : kPairs1;
         const int packed = p.ncount[i];
         const int cf = packed & 0xffff, cb = (packed >> 16) & 0xffff;
         int *tbl = tbl_base + threadIdx.x;
@@ -511,8 +508,8 @@ __device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevCo
 // error sum of R_i = max(D_i, 0) (solver_tail).
 template <bool LIST, bool DIVP, bool DYN>
 __global__ void __launch_bounds__(kBlock)
-k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
-                float *__restrict__ alpha, float4 *__restrict__ posk,
+k_density_alpha(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel,
+                float *__restrict__ alpha, float *__restrict__ rho_out, float4 *__restrict__ posk,
                 DevControl *ctl, DevStats *st, LoopHandle lh)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
@@ -562,7 +559,8 @@ k_density_alpha(PassCtx p, PV *__restrict__ pv, const float4 *__restrict__ bvel,
         float den = fmaf(Sx, Sx, fmaf(Sy, Sy, fmaf(Sz, Sz, T)));
         float a = den > 1e-6f ? rho / den : 0.0f;
         alpha[i] = a;
-        pv[i].v.w = rho;  // 4-byte store: concurrent gathers of pv[i] by other threads use xyz only
+        rho_out[i] = rho;                                          // the record's rho lane is filled by the pass that follows
+                                                                   // (other CTAs of this launch gather whole records)
         if (DIVP) {
             // Eq. 10 source (R15): R_i = max(D_i, 0), kappa^v_i = alpha_i R_i / dt
             bool on = ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0;
@@ -643,6 +641,7 @@ enum { TAIL_DIV = 0, TAIL_DENS = 1, TAIL_WCSPH = 2 };
 
 struct CTail {
     const DevControl *ctl;
+    const float *rho;         // TAIL_DIV: rho_i of this step, copied into the record's fourth velocity lane
     int add_gravity;
     const int *id;
     float4 *pos_out, *vel_out;
@@ -687,6 +686,7 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, PV *__restrict__ pv, CTai
             if (last && t.add_gravity) {
                 v.x = fmaf(dt, c.gx, v.x); v.y = fmaf(dt, c.gy, v.y); v.z = fmaf(dt, c.gz, v.z);
             }
+            v.w = t.rho[i];       // no other thread reads the records during a C-pass (it gathers posk)
             pv[i].v = v;
         } else {
             pv[i].v = v;
@@ -838,15 +838,17 @@ k_cg_direction(int n, const DevControl *__restrict__ ctl, const float4 *__restri
 // ---------------------------------------------------------------------------------------------
 // A10: WCSPH equation of state (R17): rho~ = max(rho, rho0),
 // p = k((rho~/rho0)^gamma - 1), evaluated as k expm1(gamma log1p(delta)), delta = (rho~ - rho0)/rho0,
-// which keeps the small excess accurate in fp32.  posk.w = p / rho~^2 (vel.w keeps rho).
+// which keeps the small excess accurate in fp32.  posk.w = p / rho~^2; the record's fourth velocity lane
+// receives rho (the viscosity sums gather rho_j from it).
 __global__ void __launch_bounds__(256)
-k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const PV *__restrict__ pv,
+k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const float *__restrict__ rho_in, PV *__restrict__ pv,
             float4 *__restrict__ posk)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= c.nf) return;
     float4 x = pos[i];
-    float rho = pv[i].v.w;
+    float rho = rho_in[i];
+    pv[i].v.w = rho;
     float rt = fmaxf(rho, c.rho0);
     float delta = (rt - c.rho0) / c.rho0;
     float pr = c.wc_k * expm1f(c.wc_gamma * log1pf(delta));

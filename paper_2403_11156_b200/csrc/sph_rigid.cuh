@@ -113,10 +113,11 @@ __device__ __forceinline__ void quat_to_R(const float q[4], double R[9])
     R[6] = 2 * (x * z - w * y);     R[7] = 2 * (y * z + w * x);     R[8] = 1 - 2 * (x * x + y * y);
 }
 
+// set_vel = 0 leaves the sample velocities alone (sph_write_state of positions only).
 __global__ void __launch_bounds__(256)
 k_body_rest(const float4 *__restrict__ bpos, const int *__restrict__ bbody,
             const SphRigidBody *__restrict__ bodies, int nb, float4 *__restrict__ brest,
-            float4 *__restrict__ bvel)
+            float4 *__restrict__ bvel, int set_vel)
 {
     int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nb) return;
@@ -134,7 +135,34 @@ k_body_rest(const float4 *__restrict__ bpos, const int *__restrict__ bbody,
         v.y = (float)(B.lin_vel[1] + (B.ang_vel[2] * d[0] - B.ang_vel[0] * d[2]));
         v.z = (float)(B.lin_vel[2] + (B.ang_vel[0] * d[1] - B.ang_vel[1] * d[0]));
     }
-    bvel[k] = v;
+    if (set_vel) bvel[k] = v;
+}
+
+// Samples of DYNAMIC bodies re-posed from the body states (after sph_write_state of SPH_FIELD_RIGID_BODIES):
+// x_k = X + R(q) xbar_k (set_pos), v_k = V + omega x (x_k - X) (set_vel); same arithmetic as the tail of k_rigid_step.
+__global__ void __launch_bounds__(256)
+k_body_pose(const float4 *__restrict__ brest, const int *__restrict__ bbody,
+            const SphRigidBody *__restrict__ bodies, int nb, float4 *__restrict__ bpos,
+            float4 *__restrict__ bvel, int set_pos, int set_vel)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nb) return;
+    const SphRigidBody &B = bodies[bbody[k]];
+    if (!B.dynamic) return;
+    double R[9];
+    quat_to_R(B.quat, R);
+    float4 xb = brest[k];
+    double r[3];
+    for (int a = 0; a < 3; ++a) r[a] = R[3 * a] * xb.x + R[3 * a + 1] * xb.y + R[3 * a + 2] * xb.z;
+    if (set_pos) {
+        float4 x = bpos[k];
+        x.x = (float)((double)B.com[0] + r[0]); x.y = (float)((double)B.com[1] + r[1]); x.z = (float)((double)B.com[2] + r[2]);
+        bpos[k] = x;
+    }
+    if (set_vel)
+        bvel[k] = make_float4((float)((double)B.lin_vel[0] + (double)B.ang_vel[1] * r[2] - (double)B.ang_vel[2] * r[1]),
+                              (float)((double)B.lin_vel[1] + (double)B.ang_vel[2] * r[0] - (double)B.ang_vel[0] * r[2]),
+                              (float)((double)B.lin_vel[2] + (double)B.ang_vel[0] * r[1] - (double)B.ang_vel[1] * r[0]), 0.f);
 }
 
 // Eq. 11 (R9): Psi_k = rho0 / sum_{k' in the same body, k included} W_kk'.
