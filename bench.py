@@ -92,41 +92,85 @@ def dist_env():
 
 
 # ---------------------------------------------------------------------------------------------
-# Algorithmic work per fluid particle of each kernel:
-# compulsory bytes = own inputs read once + outputs written once, neighbour gathers assumed
-# cache-served; nf / nbd = mean fluid / boundary neighbours, cand = mean candidates of the 27-cell walk.
-# Fluid list entries are 2 bytes, boundary entries 4 bytes.
-def kernel_work(name, nf_mean, nb_mean, cand_mean):
+# Algorithmic work per fluid particle of each kernel.
+#  bytes_8d   : SURVEY.md section 8(d) "compulsory HBM bytes" of the row(s) the kernel realises (own inputs read
+#               once + outputs written once, neighbours cache-served): A4 24 B, P-pass 44 B, C-pass 52 B, A9 40 B,
+#               A1-A3 ~110 B + ~10 B per cell.  The headline roofline.frac uses THIS figure.
+#  bytes_lists: the same plus what this design adds on top of 8(d): the per-step neighbour list (2 B per fluid,
+#               4 B per boundary neighbour) and the packed count word -- real traffic, but the design's own choice.
+#  nf / nbd = mean fluid / boundary neighbours, cand = mean candidates tested by the list builder.
+def kernel_work(name, nf_mean, nb_mean, cand_mean, cells_per_particle=0.0):
     lst = 2.0 * nf_mean + 4.0 * nb_mean
     nn = nf_mean + nb_mean
-    if name == "k_build_lists":        # A4 walk: pos in; count, lists out; predicate R10 on every candidate
-        return dict(bytes=16 + 4 + lst, flops=8.0 * cand_mean, row="A4 (lists)")
-    if name == "k_density_alpha":      # record, count, list in; rho, alpha, posk out (+ fused first divergence P-pass)
-        return dict(bytes=32 + 4 + lst + 4 + 4 + 16, flops=45.0 * nn + 25, row="A4 + A5 P")
-    if name == "k_solver_p":           # record, alpha, count, list in; posk out
-        return dict(bytes=32 + 4 + 4 + lst + 16, flops=27.0 * nn + 12, row="A5/A7 P")
-    if name == "k_solver_c":           # posk, count, list, vel in; vel out; one launch in three also integrates (A9)
-        return dict(bytes=16 + 4 + lst + 16 + 16 + (4 + 36) / 3.0, flops=26.0 * nn + 12, row="A5/A7 C (+A6, A9)")
-    if name == "k_reorder":            # slot, key, cell range, pos, vel, id in; pos, record, id out
-        return dict(bytes=4 + 4 + 8 + 36 + 16 + 32 + 4, flops=0.0, row="A3")
+    if name == "k_build_lists":        # first half of A4: pos in (16); lists + count out are the design's own stream
+        return dict(bytes_8d=16.0, bytes_lists=16 + 4 + lst, flops=8.0 * cand_mean, row="A4 (list build)")
+    if name == "k_density_alpha":      # A4 (pos -> rho, alpha) fused with the first P-pass of A5 (vel in, kappa/rho out)
+        return dict(bytes_8d=44.0, bytes_lists=32 + 4 + lst + 4 + 4 + 16, flops=45.0 * nn + 25, row="A4 + first A5 P")
+    if name == "k_solver_p":
+        return dict(bytes_8d=44.0, bytes_lists=32 + 4 + 4 + lst + 16, flops=27.0 * nn + 12, row="A5/A7 P")
+    if name == "k_solver_c":           # one launch in three also integrates (A9, 40 B)
+        return dict(bytes_8d=52.0 + 40.0 / 3.0, bytes_lists=16 + 4 + lst + 16 + 16 + (4 + 36) / 3.0, flops=26.0 * nn + 12,
+                    row="A5/A7 C (+A6, A9)")
+    if name in ("k_reorder", "k_sort_scatter"):
+        return dict(bytes_8d=80.0, bytes_lists=4 + 4 + 8 + 36 + 16 + 32 + 4, flops=0.0, row="A3")
     if name == "k_cell_key_hist":
-        return dict(bytes=16 + 4 + 4 + 8, flops=10.0, row="A1")
+        return dict(bytes_8d=30.0, bytes_lists=16 + 4 + 4 + 8, flops=10.0, row="A1")
     return None
 
 
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the config-4 launches in the
-# committed `ncu --set full` capture profiles/r1e_ncu_full_summary.md (another run of the same command
-# as the roofline's timing: context for `achieved`, not a live measurement)
-NCU_PROFILE = "profiles/r1e_ncu_full_summary.md"
-NCU_TRAFFIC_BYTES = {
-    ("config4_splash_1p23M", "k_solver_p"): 129.481984e6 + 4.196352e6,
-    ("config4_splash_1p23M", "k_solver_c"): 149.157376e6 + 28.326912e6,
-    ("config4_splash_1p23M", "k_build_lists"): 26.499072e6 + 27.364608e6,
-    ("config4_splash_1p23M", "k_density_alpha"): 144.392960e6 + 10.979072e6,
-}
-# l1tex__throughput.avg.pct_of_peak_sustained_active of the same capture: the list passes are bound by the
-# L1 gather path (see the profile), which is why their HBM fraction is low
-NCU_L1TEX_PCT = {"k_solver_p": 88.0, "k_solver_c": 85.5, "k_build_lists": 82.0, "k_density_alpha": 85.6}
+def step_bytes_8d(mean_it_v, mean_it_d, cells_per_particle):
+    """SURVEY 8(d) compulsory bytes of one whole DFSPH step per fluid particle (viscosity off): grid A1-A3
+    (~110 B + ~10 B per cell), A4 24, P 44 and C 52 per solver iteration, A9 40."""
+    return 110.0 + 10.0 * cells_per_particle + 24.0 + (mean_it_v + mean_it_d) * (44.0 + 52.0) + 40.0
+
+
+def csrc_sha16():
+    """Hash of the kernel sources: an ncu profile names the sources it was captured from."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2403_11156_b200", "csrc", "*.cu*"))):
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+NCU_PROFILE = "profiles/r2_ncu_full_summary.md"
+
+
+def read_ncu_profile(path=None):
+    """Parse the committed `ncu --set full` summary (a markdown table: one column per profiled launch, one row per
+    metric; a `csrc_sha16:` line names the kernel sources it was captured from).
+    Returns {kernel name: {metric: float}}, sha or None."""
+    path = os.path.join(ROOT, path or NCU_PROFILE)
+    if not os.path.exists(path):
+        return {}, None
+    sha, cols, out = None, None, {}
+    for line in open(path):
+        if line.startswith("csrc_sha16:"):
+            sha = line.split(":", 1)[1].strip().strip("`")
+        if not line.startswith("|"):
+            continue
+        cells = [c.strip() for c in line.strip().strip("|").split("|")]
+        if cells[0] == "metric":
+            cols = cells[2:]
+            for c in cols:
+                out.setdefault(c, {})
+        elif cols and not set(cells[0]) <= set("-") and len(cells) >= 2 + len(cols):
+            for c, v in zip(cols, cells[2:]):
+                try:
+                    out[c][cells[0]] = float(v.replace(",", ""))
+                except ValueError:
+                    pass
+    return out, sha
+
+
+def ncu_for_kernel(prof, name):
+    for col, m in prof.items():
+        if name in col:
+            return m
+    return None
+
+
 FINE_X = 2      # the library splits every grid cell into 2 slabs along x: x-runs cover 2.5 of the 3 cell widths
 
 
@@ -219,6 +263,31 @@ def run_ours(args):
     barrier()
     ems = max(e0.elapsed_time(e1), wall * 1e3)
     e2e_value = job_throughput(nf, Ke, max_over_ranks(ems, world, "cuda"), world)
+
+    # ---- the same metric later in the run: the driver's short default window (W + K = 25 steps) ends before
+    # the blocks of config 4 reach the obstacles (step ~75); this window starts at step >= 130, on the
+    # disordered post-impact state (reported beside the headline, not instead of it)
+    impact = None
+    if not args.no_impact_window:
+        done = int(sim.sph_read_stats()["steps_done"])
+        first = max(done, args.impact_first_step)
+        if first > done:
+            sim.sph_step_dfsph(first - done)
+        Ki = max(1, min(K, 30))
+        stA = sim.sph_read_stats()
+        barrier()
+        e0.record(stream)
+        sim.sph_step_dfsph(Ki)
+        e1.record(stream)
+        stream.synchronize()
+        barrier()
+        stB = sim.sph_read_stats()
+        ims = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+        impact = {"first_step": first, "steps": Ki, "ms_per_step": ims / Ki, "value": job_throughput(nf, Ki, ims, world),
+                  "unit": UNIT, "mean_it_v": (stB["total_it_v"] - stA["total_it_v"]) / Ki,
+                  "mean_it_d": (stB["total_it_d"] - stA["total_it_d"]) / Ki, "v_max": stB["v_max"],
+                  "err_rho_last": stB["err_rho"], "mean_fluid_neighbours": stB["mean_fluid_neighbors"],
+                  "max_fluid_neighbours": stB["max_fluid_neighbors"]}
     sim.close()
 
     out = None
@@ -241,6 +310,8 @@ def run_ours(args):
                     "steps": Ke},
             "gpu_launches": int(launches),
         }
+        if impact is not None:
+            out["impact_phase"] = impact
 
     # ---- per-kernel CUDA-event timing over the same W + K steps (host-driven launch mode: events
     # cannot bracket nodes inside a graph's WHILE body), rank 0 only -> roofline of the dominant kernel
@@ -258,38 +329,59 @@ def run_ours(args):
         sim2.sph_enable_kernel_timing(True)
         sim2.sph_step_dfsph(K)
         kt = sim2.sph_read_kernel_times()
+        sim2_ncells = sim2.ncells
         sim2.close()
         tot = sum(v[1] for v in kt.values())
         table = {k: {"launches": v[0], "ms_total": round(v[1], 3), "us_avg": round(1e3 * v[1] / v[0], 2),
                      "share": round(v[1] / tot, 4)} for k, v in sorted(kt.items(), key=lambda kv: -kv[1][1])}
         top = next(iter(table))
+        cells_pp = float(sim2_ncells) / max(nf, 1)
         work = kernel_work(top, nf_mean, nb_mean, cand_mean)
         dur = 1e-3 * kt[top][1] / kt[top][0]
         fp32_peak = N_SM * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        prof, prof_sha = read_ncu_profile()
+        stale = prof_sha is not None and prof_sha != csrc_sha16()
+        if stale:
+            sys.stderr.write("bench.py: WARNING: %s was captured from other kernel sources (csrc_sha16 %s, now %s): "
+                             "its DRAM traffic is NOT reported; re-capture it\n" % (NCU_PROFILE, prof_sha, csrc_sha16()))
+        pm = None if stale else ncu_for_kernel(prof, top)
+        traffic = (pm["dram__bytes_read.sum"] + pm["dram__bytes_write.sum"]) * 1e6 if pm and "dram__bytes_read.sum" in pm else None
         roof = {"kernel": top, "row": work["row"] if work else None, "avg_us": round(dur * 1e6, 2),
-                "share_of_step": table[top]["share"], "traffic": NCU_TRAFFIC_BYTES.get((sc.name, top)),
-                "traffic_source": NCU_PROFILE if (sc.name, top) in NCU_TRAFFIC_BYTES else None,
-                "l1tex_throughput_pct_ncu": NCU_L1TEX_PCT.get(top),
+                "share_of_step": table[top]["share"], "traffic": traffic,
+                "traffic_source": NCU_PROFILE if traffic is not None else None,
+                "l1tex_throughput_pct_ncu": pm.get("l1tex__throughput.avg.pct_of_peak_sustained_active") if pm else None,
+                "issue_active_pct_ncu": pm.get("smsp__issue_active.avg.pct_of_peak_sustained_active") if pm else None,
                 "peak_source": peaks["source"] + " (MEASURED_PEAKS.json)"}
         if work:
-            gbs = work["bytes"] * nf / dur / 1e9
+            gbs = work["bytes_8d"] * nf / dur / 1e9
+            gbs_l = work["bytes_lists"] * nf / dur / 1e9
             tfl = work["flops"] * nf / dur / 1e12
-            roof["algorithmic_bytes"] = work["bytes"] * nf
-            if top == "k_build_lists":
-                roof.update({"bound": "alu", "achieved": tfl, "peak": fp32_peak, "unit": "TFLOP/s",
-                             "frac": tfl / fp32_peak, "hbm_achieved_gbs": gbs, "hbm_frac": gbs / peaks["hbm_gbs"]})
-            else:
-                roof.update({"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                             "frac": gbs / peaks["hbm_gbs"], "alu_achieved_tflops": tfl, "alu_frac": tfl / fp32_peak})
+            roof.update({"bound": "hbm", "algorithmic_bytes": work["bytes_8d"] * nf,
+                         "algorithmic_bytes_per_particle": work["bytes_8d"],
+                         "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": gbs / peaks["hbm_gbs"],
+                         "frac_with_lists": gbs_l / peaks["hbm_gbs"], "bytes_with_lists_per_particle": work["bytes_lists"],
+                         "traffic_over_algorithmic": (traffic / (work["bytes_8d"] * nf)) if traffic else None,
+                         "alu_achieved_tflops": tfl, "alu_frac": tfl / fp32_peak,
+                         "note": "frac = SURVEY 8(d) compulsory bytes / event-timed duration / measured HBM peak; the list "
+                                 "passes are bound by L1 gather wavefronts and instruction issue (see l1tex / issue figures), "
+                                 "not by HBM"})
+        sb = step_bytes_8d(mean_it_v, mean_it_d, cells_pp) * nf
+        out["roofline_step"] = {"bound": "hbm", "algorithmic_bytes": sb, "achieved": sb / (ms_max / K * 1e-3) / 1e9,
+                                "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                "frac": sb / (ms_max / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                "what": "SURVEY 8(d) bytes of the whole step / ms_per_step"}
         per_kernel = {}
         for k in table:
             w = kernel_work(k, nf_mean, nb_mean, cand_mean)
             if w:
                 d = 1e-3 * kt[k][1] / kt[k][0]
+                km = None if stale else ncu_for_kernel(prof, k)
                 per_kernel[k] = {"row": w["row"], "us_avg": table[k]["us_avg"], "share": table[k]["share"],
-                                 "hbm_gbs": round(w["bytes"] * nf / d / 1e9, 1),
-                                 "hbm_frac": round(w["bytes"] * nf / d / 1e9 / peaks["hbm_gbs"], 4),
-                                 "fp32_tflops": round(w["flops"] * nf / d / 1e12, 2)}
+                                 "hbm_frac": round(w["bytes_8d"] * nf / d / 1e9 / peaks["hbm_gbs"], 4),
+                                 "hbm_frac_with_lists": round(w["bytes_lists"] * nf / d / 1e9 / peaks["hbm_gbs"], 4),
+                                 "fp32_tflops": round(w["flops"] * nf / d / 1e12, 2),
+                                 "dram_bytes_ncu": ((km["dram__bytes_read.sum"] + km["dram__bytes_write.sum"]) * 1e6
+                                                    if km and "dram__bytes_read.sum" in km else None)}
         out["roofline"] = roof
         out["kernels"] = per_kernel
         out["kernel_time_table"] = table
@@ -388,6 +480,8 @@ def main():
                     help="scaling sweep: config-4 scene proportions at this many fluid particles (250e3 / 4e6 / 8e6); "
                          "not the headline line")
     ap.add_argument("--no-breakdown", action="store_true")
+    ap.add_argument("--no-impact-window", action="store_true")
+    ap.add_argument("--impact-first-step", type=int, default=130)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":

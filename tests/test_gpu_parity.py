@@ -407,11 +407,17 @@ def _drop_block_onto_bodies(B, g, sc, speed=3.0):
     the rigid step then act from the first step on."""
     import torch
     bp = g.sph_read_state(B.BOUNDARY_POS)
-    dyn = torch.zeros(g.nb, dtype=torch.bool, device="cuda")
-    for b in sc.bodies:
-        if b.dynamic:
-            dyn[b.first_particle:b.first_particle + b.n_particles] = True
-    top = float(bp[dyn][:, 2].max())
+    tops = {i: float(bp[b.first_particle:b.first_particle + b.n_particles, 2].max())
+            for i, b in enumerate(sc.bodies) if b.dynamic}
+    top = max(tops.values())
+    # lift the lower bodies (through SPH_FIELD_RIGID_BODIES) until all tops are level: every body is hit at once
+    newb = []
+    for i, b in enumerate(g.read_bodies()):
+        nb_ = scenes.Body(**b)
+        if b["dynamic"]:
+            nb_.com = (b["com"][0], b["com"][1], b["com"][2] + (top - tops[i]))
+        newb.append(nb_)
+    g.sph_write_state(B.RIGID_BODIES, newb)
     p0 = g.sph_read_state(B.POS).clone()
     s = 2.0 * sc.params["particle_radius"]
     p0[:, 2] -= float(p0[:, 2].min()) - (top + s)
