@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 LIB = os.path.join(_HERE, "libsph_b200.so")
 SOURCES = [os.path.join(_HERE, "csrc", "sph_api.cu")]
-DEPS = glob.glob(os.path.join(_HERE, "csrc", "*")) + [os.path.join(_ROOT, "include", "sph.h")]
+DEPS = glob.glob(os.path.join(_HERE, "csrc", "*.cu*")) + [os.path.join(_ROOT, "include", "sph.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -35,7 +35,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + SOURCES
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("SPH_NVCC_EXTRA", "").split() + ["-o", LIB] + SOURCES
         res = subprocess.run(cmd, capture_output=True, text=True)
         log = os.path.join(_HERE, "csrc", "build.log")
         with open(log, "w") as f:

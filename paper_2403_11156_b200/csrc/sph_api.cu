@@ -12,6 +12,7 @@
 #include "sph_common.cuh"
 #include "sph_grid.cuh"
 #include "sph_passes.cuh"
+#include "sph_lists.cuh"
 #include "sph_rigid.cuh"
 
 using namespace sph;
@@ -53,6 +54,7 @@ struct SphSim {
     size_t cs_len = 0;              // ncells + 1 rounded up to 4
     // fluid store
     float4 *posA = nullptr, *velA = nullptr, *posB = nullptr, *posk = nullptr;
+    float *px = nullptr, *py = nullptr, *pz = nullptr;   // sorted positions, structure of arrays (+ 4 floats of padding)
     PV *pvB = nullptr, *pvC = nullptr;   // { pos | vel, rho } records of the passes; pvC: output of explicit viscosity
     int *idA = nullptr, *idB = nullptr;
     float *alpha = nullptr, *rho = nullptr;
@@ -226,7 +228,9 @@ size_t layout(SphSim &s, void *base)
     s.ctl = w.take<DevControl>(1);
     s.stats = w.take<DevStats>(1);
     s.posA = w.take<float4>(nf1); s.velA = w.take<float4>(nf1); s.idA = w.take<int>(nf1);
-    s.posB = w.take<float4>(nf1 + kPosPad); s.pvB = w.take<PV>(nf1); s.idB = w.take<int>(nf1);
+    s.posB = w.take<float4>(nf1);
+    s.px = w.take<float>(nf1 + 4); s.py = w.take<float>(nf1 + 4); s.pz = w.take<float>(nf1 + 4);
+    s.pvB = w.take<PV>(nf1); s.idB = w.take<int>(nf1);
     s.pvC = s.prm.viscosity_mode == 1 ? w.take<PV>(nf1) : nullptr;
     s.posk = w.take<float4>(nf1);
     s.alpha = w.take<float>(nf1);
@@ -277,9 +281,9 @@ int enqueue_grid(SphSim *s, cudaStream_t st, GridBufs &g, const float4 *a_in, co
     if (g.n > 0) {
         LAUNCH(s, k_scatter_slots, cdiv(g.n, 256), 256, st, g.key, g.off, g.cell_start, g.n, g.slot);
         if (fluid) LAUNCH(s, k_reorder<true>, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
-                          a_out, b_out, id_out);
+                          a_out, b_out, id_out, s->px, s->py, s->pz);
         else       LAUNCH(s, k_reorder<false>, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
-                          a_out, b_out, id_out);
+                          a_out, b_out, id_out, (float *)nullptr, (float *)nullptr, (float *)nullptr);
     }
     return SPH_OK;
 }
@@ -341,12 +345,11 @@ int enqueue_fluid_grid_and_lists(SphSim *s, cudaStream_t st)
     if (rc) return rc;
     if (s->c.nf > 0) {
         PassCtx p = make_ctx(s);
-        // staging rows of the list builder: kf + kStageExtra rows of 32 16-bit entries per warp
-        const int rows = s->c.kf + kStageExtra;
-        const size_t smem = (size_t)rows * 64 * (kBlock / 32);
+        const BuildShape bs = build_shape(s->c.kf);
+        const int grid = cdiv(s->c.nf, 64 * bs.warps);
         cudaEvent_t ea_ = nullptr, eb_ = nullptr;
         if (s->timing) { ea_ = take_event(s); eb_ = take_event(s); cudaEventRecord(ea_, st); }
-        k_build_lists<<<s->nblocks, kBlock, smem, st>>>(p, &s->stats->lc, rows);
+        k_build_lists<<<grid, 32 * bs.warps, bs.smem, st>>>(p, s->px, s->py, s->pz, &s->stats->lc, bs.rows);
         if (s->timing) { cudaEventRecord(eb_, st); s->timed.push_back({ "k_build_lists", ea_, eb_ }); }
         ++*s->cur_counter;
         CUDA_TRY(s, cudaGetLastError());
@@ -773,8 +776,11 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
             CARVE((k_cg_apply<true, true>)); CARVE((k_cg_apply<true, false>));
 #undef CARVE
         }
-        CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (kMaxListCap + kStageExtra) * 64 * (kBlock / 32)));
+        CUDA_TRY(s, cudaFuncSetAttribute(k_build_lists, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)build_shape(s->c.kf).smem));
+        // the SoA arrays are read up to 3 elements past the last particle (16-byte granules of the bulk copies)
+        CUDA_TRY(s, cudaMemsetAsync(s->px + s->c.nf, 0, 4 * sizeof(float), s->stream));
+        CUDA_TRY(s, cudaMemsetAsync(s->py + s->c.nf, 0, 4 * sizeof(float), s->stream));
+        CUDA_TRY(s, cudaMemsetAsync(s->pz + s->c.nf, 0, 4 * sizeof(float), s->stream));
         const int nf = s->c.nf, nb = s->c.nb;
         // control + statistics blocks
         DevControl hc;

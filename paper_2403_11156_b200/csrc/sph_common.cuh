@@ -68,7 +68,8 @@ struct DevControl {
 
 // Statistics block in device memory; sph_read_stats copies it out and converts to SphStats.
 struct ListCounters {
-    int overflow, max_f, max_b, pad;
+    int max_f, max_b;            // read together (one 8-byte load) by the list builder's guard
+    int overflow, pad;
     unsigned long long sum_f;
 };
 struct DevStats {

@@ -166,7 +166,7 @@ k_scatter_slots(const int *__restrict__ key, const int *__restrict__ off,
 // previous sorted store, R12: makes the run bit-reproducible although the histogram atomics are
 // not), then gather of every persistent field into sorted order.
 // For the fluid store (FLUID): a = pos(x,y,z,-), b = vel(vx,vy,vz,-), ids carried; a_out = packed
-// positions, b_out = { pos | vel } records.
+// positions, b_out = { pos | vel } records, (sx, sy, sz) = structure-of-arrays positions.
 // For the boundary store: a = (x,y,z,psi), b = (vx,vy,vz,-), ids = original boundary index.
 template <bool FLUID>
 __global__ void __launch_bounds__(256)
@@ -174,7 +174,7 @@ k_reorder(const int *__restrict__ slot_src, const int *__restrict__ key,
           const int *__restrict__ cell_start, int n,
           const float4 *__restrict__ a_in, const float4 *__restrict__ b_in,
           const int *__restrict__ id_in, float4 *__restrict__ a_out, float4 *__restrict__ b_out,
-          int *__restrict__ id_out)
+          int *__restrict__ id_out, float *__restrict__ sx, float *__restrict__ sy, float *__restrict__ sz)
 {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
@@ -194,6 +194,7 @@ k_reorder(const int *__restrict__ slot_src, const int *__restrict__ key,
         // b_out is the 32-byte record array { pos | vel } of the passes (PV in sph_passes.cuh)
         b_out[2 * dst] = a;
         b_out[2 * dst + 1] = b_in[src];
+        sx[dst] = a.x; sy[dst] = a.y; sz[dst] = a.z;     // SoA copy: what the list builder bulk-copies into its tiles
     } else if (b_in != nullptr) b_out[dst] = b_in[src];
     id_out[dst] = id_in != nullptr ? id_in[src] : src;
 }

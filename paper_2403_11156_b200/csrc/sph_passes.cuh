@@ -235,169 +235,6 @@ __device__ __forceinline__ float pair_gradf(const SimConst &c, float d2)
 }
 
 // ---------------------------------------------------------------------------------------------
-// A4 first half: ONE walk of the 27 cells per particle per step evaluates the neighbour predicate
-// (R10, bit-exact) and writes the neighbour lists every pass of the step gathers through.  The
-// walk tests ~209 candidates to find ~30 neighbours, so its loop body is kept to the test, a
-// predicated 2-byte shared-memory store and a predicated pointer bump; all arithmetic on
-// neighbours happens in the list passes.
-//  * candidates of an x-run are contiguous, so two of them arrive per 256-bit load
-//    (LDG.E.256, sm_100): half the L1 wavefronts and load instructions of one float4 per candidate;
-//    the pair containing the run's first / last element may reach one element outside the run,
-//    which the range test (unsigned)(j - s) < e - s rejects (pos is padded by kPosPad elements);
-//  * list entries are staged in a per-lane shared-memory column (row k of lane l at
-//    stage[k * 32 + l]) and copied out as 32-bit words, one coalesced 128-byte row per warp store,
-//    instead of one partial-sector global store per entry.
-constexpr int kPosPad = 4;         // float4 elements readable past pos[nf - 1]
-constexpr int kStageExtra = 8;     // staging rows beyond kf.  Small on purpose: the builder's occupancy is set by this buffer
-                                   // (32 extra rows: 9 CTAs per SM, 207 us; 8: 10 CTAs, 198 us); a run that may not fit
-                                   // takes the guarded loop
-constexpr int kMaxListCap = 768;   // (kMaxListCap + kStageExtra) * 64 B * 4 warps <= 227 KB of shared memory
-
-__device__ __forceinline__ void sts_u16(uint32_t addr, int v)
-{
-    asm volatile("st.shared.u16 [%0], %1;" :: "r"(addr), "h"((unsigned short)v) : "memory");
-}
-__device__ __forceinline__ uint32_t lds_u16(uint32_t addr)
-{
-    unsigned short v;
-    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
-    return v;
-}
-
-// One x-run [s, s + len) of fluid candidates for particle i at xi.  SELF: the run contains i itself.
-// GUARD = false: the caller guarantees cf + len <= rows.  Returns the new entry count.
-template <bool SELF, bool GUARD>
-__device__ __forceinline__ int build_run(const float4 *__restrict__ pos, float4 xi, float h2, int i, int s,
-                                         int len, int tag, uint32_t st /* shared address of row 0 */, int cf, int rows)
-{
-    const int j0 = s & ~1;
-    const float4 *pp = pos + j0;
-    int off = j0 - s;                               // offset of the pair's first element: -1 or 0
-    const unsigned ulen = (unsigned)len;
-    const int self_off = i - s;
-    uint32_t w = st + cf * 64;                      // rows are 32 lanes x 2 bytes apart
-    auto test = [&](const float4 &q, int o) {
-        float dx = __fsub_rn(xi.x, q.x), dy = __fsub_rn(xi.y, q.y), dz = __fsub_rn(xi.z, q.z);
-        float d2 = dist2_r10(dx, dy, dz);
-        bool hit = d2 < h2 && (unsigned)o < ulen;
-        if (SELF) hit = hit && o != self_off;
-        if (GUARD) {
-            if (hit) { if (cf < rows) sts_u16(st + cf * 64, tag + o); ++cf; }
-        } else {
-            if (hit) { sts_u16(w, tag + o); w += 64; }
-        }
-    };
-    // software pipeline: the two pairs of the next iteration are in flight while this one is tested
-    float4 a0, a1, b0, b1;
-    ldg256(pp, a0, a1);
-    ldg256(pp + 2, b0, b1);
-#pragma unroll 1
-    for (; off < len; off += 4) {
-        pp += 4;
-        float4 c0 = a0, c1 = a1, d0 = b0, d1 = b1;
-        if (off + 4 < len) {
-            ldg256(pp, a0, a1);
-            ldg256(pp + 2, b0, b1);
-        }
-        test(c0, off); test(c1, off + 1); test(d0, off + 2); test(d1, off + 3);
-    }
-    return GUARD ? cf : (int)((w - st) >> 6);
-}
-
-__global__ void __launch_bounds__(kBlock)
-k_build_lists(PassCtx p, ListCounters *__restrict__ lc, int rows)
-{
-    extern __shared__ __align__(16) uint16_t stage_all[];      // [kBlock / 32][rows][32]
-    const SimConst &c = p.c;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
-    const uint32_t st = (uint32_t)__cvta_generic_to_shared(stage_all) + ((threadIdx.x >> 5) * rows * 32 + lane) * 2;
-    int cf = 0, cb = 0;
-    bool ovf = false;
-    if (i < c.nf) {
-        const float4 xi = p.pos[i];
-        const CellOf cell = cell_of(c.g, xi.x, xi.y, xi.z);
-        const float h2 = c.h2;
-        // the cell_start words of run r + 1 are requested before run r is walked
-        auto run_range = [&](int r, int &s, int &len) {
-            int first;
-            s = 0; len = 0;
-            if (r < kRows && run_first_cell(c.g, cell, r, first)) {
-                s = __ldg(p.fcs + first);
-                len = __ldg(p.fcs + first + (cell.x1 - cell.x0) + 1) - s;
-            }
-        };
-        int s_next, len_next;
-        run_range(0, s_next, len_next);
-#pragma unroll 1
-        for (int r = 0; r < kRows; ++r) {
-            const int s = s_next;
-            int len = len_next;
-            run_range(r + 1, s_next, len_next);
-            if (len <= 0) continue;
-            if (len > kOffMask + 1) { ovf = true; len = kOffMask + 1; }      // offsets are 12-bit
-            const int tag = r << kOffBits;
-            if (cf + len <= rows) {
-                cf = r == 4 ? build_run<true, false>(p.pos, xi, h2, i, s, len, tag, st, cf, rows)
-                            : build_run<false, false>(p.pos, xi, h2, i, s, len, tag, st, cf, rows);
-            } else {
-                cf = r == 4 ? build_run<true, true>(p.pos, xi, h2, i, s, len, tag, st, cf, rows)
-                            : build_run<false, true>(p.pos, xi, h2, i, s, len, tag, st, cf, rows);
-            }
-        }
-        // copy-out: word k of the tile row = entries (2k, 2k + 1) of this lane (layout of list_tile)
-        {
-            const int n = min(cf, c.kf);
-            uint32_t *dst = reinterpret_cast<uint32_t *>(p.nl_f + list_tile(i, c.kf)) + lane;
-            for (int k = 0; k < n; k += 2) {
-                uint32_t lo = lds_u16(st + k * 64), hi = k + 1 < n ? lds_u16(st + (k + 1) * 64) : 0u;
-                dst[(k >> 1) * 32] = lo | (hi << 16);
-            }
-        }
-        if (c.nb > 0) {
-            int *lb = p.nl_b + list_tile(i, c.kb) + lane;
-            for_each_candidate(c.g, p.bcs, cell, [&](int k, int, int) {
-                float4 q = __ldg(p.bpos + k);
-                float dx = __fsub_rn(xi.x, q.x), dy = __fsub_rn(xi.y, q.y), dz = __fsub_rn(xi.z, q.z);
-                float d2 = dist2_r10(dx, dy, dz);
-                if (d2 < h2) {
-                    if (cb < c.kb) lb[cb * 32] = k;
-                    ++cb;
-                }
-            });
-        }
-        p.ncount[i] = min(cf, c.kf) | (min(cb, c.kb) << 16);
-        ovf = ovf || cf > c.kf || cb > c.kb;
-    }
-    // statistics: overflow count, maxima, neighbour-count sum.  Same-address atomics serialise in
-    // L2, so the maxima are guarded by a plain read (they only grow) and the sums go through one
-    // shared-memory reduction and one atomic per CTA.
-    __shared__ int red_i[2 * (kBlock / 32)];
-    unsigned bo = __ballot_sync(0xffffffffu, ovf);
-    int mf = cf, mb = cb, sf = cf;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        mf = max(mf, __shfl_xor_sync(0xffffffffu, mf, o));
-        mb = max(mb, __shfl_xor_sync(0xffffffffu, mb, o));
-        sf += __shfl_xor_sync(0xffffffffu, sf, o);
-    }
-    if (lane == 0) {
-        if (mf > *(volatile int *)&lc->max_f) atomicMax(&lc->max_f, mf);
-        if (mb > *(volatile int *)&lc->max_b) atomicMax(&lc->max_b, mb);
-        red_i[threadIdx.x >> 5] = sf;
-        red_i[kBlock / 32 + (threadIdx.x >> 5)] = __popc(bo);
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int ts = 0, to = 0;
-#pragma unroll
-        for (int w = 0; w < kBlock / 32; ++w) { ts += red_i[w]; to += red_i[kBlock / 32 + w]; }
-        atomicAdd(&lc->sum_f, (unsigned long long)ts);
-        if (to) atomicAdd(&lc->overflow, to);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
 // A12: device-side reductions and loop control.  Every P-pass reduces its error term on the
 // device; the LAST CTA of the launch to finish evaluates the loop predicate of Alg. 2
 // (R14: the error measured by this iteration's P-pass decides whether another
