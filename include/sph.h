@@ -199,7 +199,8 @@ int sph_set_forced_iterations(SphSim *sim, int forced_v, int forced_d, int force
  * size.  is_host = 0: dst/src is a device pointer, copy is asynchronous on the stream;
  * is_host = 1: host pointer, the call returns after the copy has completed.
  * sph_write_state (any writable field) invalidates grid-derived fields until the next
- * sph_build_grid / step.  Boundary fields take effect at that next sph_build_grid / step call:
+ * sph_build_grid / step.  Boundary fields take effect at that next sph_build_grid / step call (or at the next
+ * sph_read_state of a boundary / body field, which then already shows the re-posed samples):
  *   SPH_FIELD_BOUNDARY_POS : the samples' world positions are replaced; their body-frame coordinates
  *                            (pose of their body as it is then) and the Akinci volumes Psi_k (Eq. 11,
  *                            PAPER.md:178) are recomputed; the sorted boundary store is rebuilt;

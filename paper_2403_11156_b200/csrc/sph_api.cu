@@ -884,6 +884,8 @@ int sph_read_state(SphSim *s, int field, void *dst, size_t bytes, int is_host)
     if (bytes > 0 && !dst) { s->err = "dst is NULL"; return SPH_EINVAL; }
     if (fi.derived && !s->derived_valid) { s->err = "field is stale: call sph_build_grid or a step first"; return SPH_ESTATE; }
     DeviceGuard dg(s->device);
+    // pending boundary / body writes become visible to reads as well (samples re-posed, Psi recomputed)
+    if (s->boundary_dirty && field >= SPH_FIELD_BOUNDARY_POS) { int rc = refresh_boundary(s); if (rc) return rc; }
     if (!is_host) return export_field(s, field, dst, bytes);
     if (bytes > s->staging_bytes) { s->err = "field too large for a host read; read it into a device buffer"; return SPH_EINVAL; }
     int rc = export_field(s, field, s->staging, bytes);
