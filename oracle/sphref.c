@@ -61,6 +61,9 @@ typedef struct SphRefParams {
     double wcsph_stiffness, wcsph_exponent;
     double cfl_factor;          /* lambda of reading R26; 0 => fixed dt */
     double dt_min;
+    int warm_start;             /* reading R27: 1 => both DFSPH solves start from the stiffness applied in the last step */
+    double warm_start_factor;   /* omega of reading R27 (0.5 in the cited source's public implementation) */
+    int pcisph_min_iter, pcisph_max_iter;   /* reading R28 */
 } SphRefParams;
 
 typedef struct SphRefBody {
@@ -97,6 +100,9 @@ typedef struct SphRef {
     int *bbody;
     SphRefBody *bodies;
     double *rho, *alpha, *kappa, *kr; /* [nf] */
+    double *ksum_v, *ksum_d; /* [nf] total stiffness applied by the divergence / density solve of the last step (R27) */
+    double *kacc;            /* [nf] scratch: running total of the solve in progress */
+    double pci_delta;        /* PCISPH scaling factor (R28), computed at creation */
     double *vstar;       /* scratch */
     CellList gf, gb;     /* fluid grid, boundary grid */
     int *nf_start, *nf_idx; /* CSR fluid neighbours of fluid i */
@@ -346,6 +352,8 @@ SphRef *sphref_create(const SphRefParams *p, int nf, const float *fpos, const fl
     s->vstar = (double *)calloc(f3, sizeof(double));
     s->rho = (double *)calloc(f3, sizeof(double)); s->alpha = (double *)calloc(f3, sizeof(double));
     s->kappa = (double *)calloc(f3, sizeof(double)); s->kr = (double *)calloc(f3, sizeof(double));
+    s->ksum_v = (double *)calloc(f3, sizeof(double)); s->ksum_d = (double *)calloc(f3, sizeof(double));
+    s->kacc = (double *)calloc(f3, sizeof(double));
     s->bx = (double *)calloc(b3, sizeof(double)); s->bv = (double *)calloc(b3, sizeof(double));
     s->brest = (double *)calloc(b3, sizeof(double)); s->bforce = (double *)calloc(b3, sizeof(double));
     s->psi = (double *)calloc(b3, sizeof(double));
@@ -375,6 +383,7 @@ void sphref_destroy(SphRef *s)
 {
     if (!s) return;
     free(s->x); free(s->v); free(s->vstar); free(s->rho); free(s->alpha); free(s->kappa); free(s->kr);
+    free(s->ksum_v); free(s->ksum_d); free(s->kacc);
     free(s->bx); free(s->bv); free(s->brest); free(s->bforce); free(s->psi); free(s->bbody); free(s->bodies);
     free(s->nf_start); free(s->nf_idx); free(s->nb_start); free(s->nb_idx); free(s->cg_hist);
     celllist_free(&s->gf); celllist_free(&s->gb);
@@ -485,6 +494,25 @@ static void apply_pressure_update(SphRef *s, double *vel)
     memcpy(vel, s->vstar, sizeof(double) * 3 * (size_t)s->nf);
 }
 
+/* Warm start (reading R27; PAPER.md:49, 170 only say that the PPE solvers need fewer refinement rounds / allow larger
+ * steps -- the technique is the one of the cited DFSPH source [5]): before a solve's loop, the total stiffness K_i that
+ * the same solve applied in the LAST step, scaled by omega, is applied once through the ordinary pressure update,
+ *   v <- v - dt U[omega K / rho]   (rho, gradW of the CURRENT step),
+ * and the solve's running total starts from it: K_i(new) = omega K_i(old) + sum over this step's iterations of kappa_i.
+ * Returns with s->kacc initialised (zeros when warm start is off). */
+static void warm_start_apply(SphRef *s, double *vel, const double *ksum_prev)
+{
+    const SphRefParams *p = &s->p;
+    for (int i = 0; i < s->nf; ++i) s->kacc[i] = 0.0;
+    if (!p->warm_start) return;
+    for (int i = 0; i < s->nf; ++i) {
+        s->kappa[i] = p->warm_start_factor * ksum_prev[i];
+        s->kr[i] = s->kappa[i] / s->rho[i];
+        s->kacc[i] = s->kappa[i];
+    }
+    apply_pressure_update(s, vel);
+}
+
 /* Divergence-free solve, (c.2) step 3 (Eq. 10 source term PAPER.md:156; loop Alg. 2
  * PAPER.md:160-168; details from cited [5], readings R5, R14, R15):
  * do { P: R_i = max(D_i[v], 0); err_v = (dt/rho0) mean R_i; kappa^v_i = alpha_i R_i / dt;
@@ -495,7 +523,8 @@ int sphref_divergence_solve(SphRef *s, double *vel, int forced)
     const SphRefParams *p = &s->p;
     int l = 0;
     double err = 0.0;
-    if (forced == 0) { s->stats.it_v = 0; s->stats.err_v = 0.0; return 0; }
+    if (forced == 0) { s->stats.it_v = 0; s->stats.err_v = 0.0; for (int i = 0; i < s->nf; ++i) s->ksum_v[i] = 0.0; return 0; }
+    warm_start_apply(s, vel, s->ksum_v);
     for (;;) {
         double sum = 0.0;
 #pragma omp parallel for schedule(dynamic, 256) reduction(+ : sum)
@@ -505,6 +534,7 @@ int sphref_divergence_solve(SphRef *s, double *vel, int forced)
             sum += R;
             s->kappa[i] = s->alpha[i] * R / p->dt;
             s->kr[i] = s->kappa[i] / s->rho[i];
+            s->kacc[i] += s->kappa[i];
         }
         err = s->nf > 0 ? p->dt / p->rest_density * sum / s->nf : 0.0;
         apply_pressure_update(s, vel);
@@ -513,6 +543,7 @@ int sphref_divergence_solve(SphRef *s, double *vel, int forced)
         else if (!((err > p->eta_divergence || l < p->min_iter_divergence) && l < p->max_iter_divergence)) break;
     }
     s->stats.it_v = l; s->stats.err_v = err;
+    memcpy(s->ksum_v, s->kacc, sizeof(double) * (size_t)s->nf);
     return l;
 }
 
@@ -525,7 +556,8 @@ int sphref_density_solve(SphRef *s, double *vel, int forced)
     const SphRefParams *p = &s->p;
     int l = 0;
     double err = 0.0;
-    if (forced == 0) { s->stats.it_d = 0; s->stats.err_rho = 0.0; return 0; }
+    if (forced == 0) { s->stats.it_d = 0; s->stats.err_rho = 0.0; for (int i = 0; i < s->nf; ++i) s->ksum_d[i] = 0.0; return 0; }
+    warm_start_apply(s, vel, s->ksum_d);
     for (;;) {
         double sum = 0.0;
 #pragma omp parallel for schedule(dynamic, 256) reduction(+ : sum)
@@ -535,6 +567,7 @@ int sphref_density_solve(SphRef *s, double *vel, int forced)
             sum += E;
             s->kappa[i] = s->alpha[i] * E / (p->dt * p->dt);
             s->kr[i] = s->kappa[i] / s->rho[i];
+            s->kacc[i] += s->kappa[i];
         }
         err = s->nf > 0 ? sum / s->nf / p->rest_density : 0.0;
         apply_pressure_update(s, vel);
@@ -543,6 +576,7 @@ int sphref_density_solve(SphRef *s, double *vel, int forced)
         else if (!((err > p->eta_density || l < p->min_iter_density) && l < p->max_iter_density)) break;
     }
     s->stats.it_d = l; s->stats.err_rho = err;
+    memcpy(s->ksum_d, s->kacc, sizeof(double) * (size_t)s->nf);
     return l;
 }
 
@@ -828,6 +862,13 @@ double *sphref_density(SphRef *s) { return s->rho; }
 double *sphref_alpha(SphRef *s) { return s->alpha; }
 double *sphref_kappa(SphRef *s) { return s->kappa; }
 double *sphref_kr(SphRef *s) { return s->kr; }
+double *sphref_ksum_v(SphRef *s) { return s->ksum_v; }
+double *sphref_ksum_d(SphRef *s) { return s->ksum_d; }
+void sphref_set_warm_state(SphRef *s, const double *kv, const double *kd)
+{
+    memcpy(s->ksum_v, kv, sizeof(double) * (size_t)s->nf);
+    memcpy(s->ksum_d, kd, sizeof(double) * (size_t)s->nf);
+}
 double *sphref_psi(SphRef *s) { return s->psi; }
 double *sphref_boundary_pos(SphRef *s) { return s->bx; }
 double *sphref_boundary_vel(SphRef *s) { return s->bv; }

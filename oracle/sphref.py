@@ -42,7 +42,13 @@ class Params(C.Structure):
         ("enable_divergence_solve", C.c_int), ("force_iterations", C.c_int),
         ("wcsph_stiffness", C.c_double), ("wcsph_exponent", C.c_double),
         ("cfl_factor", C.c_double), ("dt_min", C.c_double),
+        ("warm_start", C.c_int), ("warm_start_factor", C.c_double),
+        ("pcisph_min_iter", C.c_int), ("pcisph_max_iter", C.c_int),
     ]
+
+
+# parameters that scenes need not spell out
+_DEFAULTS = dict(cfl_factor=0.0, dt_min=0.0, warm_start=0, warm_start_factor=0.5, pcisph_min_iter=3, pcisph_max_iter=100)
 
 
 class Body(C.Structure):
@@ -92,8 +98,10 @@ def lib():
         L.sphref_set_bodies.argtypes = [C.c_void_p, C.POINTER(Body)]
         L.sphref_get_bodies.argtypes = [C.c_void_p, C.POINTER(Body)]
         L.sphref_set_params.argtypes = [C.c_void_p, C.POINTER(Params)]
+        L.sphref_set_warm_state.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.sphref_set_warm_state.restype = None
         for name in ("sphref_pos", "sphref_vel", "sphref_density", "sphref_alpha", "sphref_kappa",
-                     "sphref_kr", "sphref_psi", "sphref_boundary_pos", "sphref_boundary_vel",
+                     "sphref_kr", "sphref_ksum_v", "sphref_ksum_d", "sphref_psi", "sphref_boundary_pos", "sphref_boundary_vel",
                      "sphref_boundary_force"):
             getattr(L, name).argtypes = [C.c_void_p]
             getattr(L, name).restype = dp
@@ -133,7 +141,7 @@ def num_threads() -> int:
 def make_params(prm: Dict[str, object]) -> Params:
     p = Params()
     for name, ctype in Params._fields_:
-        val = prm.get(name, 0.0) if name in ("cfl_factor", "dt_min") else prm[name]
+        val = prm.get(name, _DEFAULTS[name]) if name in _DEFAULTS else prm[name]
         if hasattr(ctype, "_length_"):
             setattr(p, name, ctype(*[float(v) for v in val]))
         else:
@@ -291,6 +299,15 @@ class Sim:
     def density(self): return self._arr(lib().sphref_density, self.nf)
     def alpha(self): return self._arr(lib().sphref_alpha, self.nf)
     def kappa(self): return self._arr(lib().sphref_kappa, self.nf)
+    def ksum_v(self): return self._arr(lib().sphref_ksum_v, self.nf)
+    def ksum_d(self): return self._arr(lib().sphref_ksum_d, self.nf)
+
+    def set_warm_state(self, ksum_v, ksum_d):
+        """Total stiffness of the last step's divergence / density solve (reading R27), id order."""
+        a = np.ascontiguousarray(ksum_v, dtype=np.float64)
+        b = np.ascontiguousarray(ksum_d, dtype=np.float64)
+        assert a.shape == (self.nf,) and b.shape == (self.nf,)
+        lib().sphref_set_warm_state(self._h, a.ctypes.data, b.ctypes.data)
     def psi(self): return self._arr(lib().sphref_psi, self.nb) if self.nb else np.zeros(0)
     def boundary_pos(self): return self._arr(lib().sphref_boundary_pos, self.nb, 3) if self.nb else np.zeros((0, 3))
     def boundary_vel(self): return self._arr(lib().sphref_boundary_vel, self.nb, 3) if self.nb else np.zeros((0, 3))
