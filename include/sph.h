@@ -37,7 +37,7 @@
 extern "C" {
 #endif
 
-#define SPH_ABI_VERSION 1
+#define SPH_ABI_VERSION 2
 
 typedef enum SphError {
     SPH_OK = 0,
@@ -88,6 +88,13 @@ typedef struct SphParams {
                                   dt = clamp(lambda 2r / max_i |v_i|, dt_min, dt) with the velocities at the
                                   step's start (reading R26); 0: fixed dt */
     float dt_min;
+    int   warm_start;          /* 1: both DFSPH solves start from the stiffness applied in the last step (reading R27;
+                                  SURVEY 8(f) NEXT-1): before each loop one C-pass applies
+                                  omega K_i, K_i = total kappa_i of that solve in the previous step, carried with the
+                                  particle through the sort.  Costs one C-pass per solve (and un-fuses the first
+                                  divergence P-pass); pays when the loops run well above their minimum counts */
+    float warm_start_factor;   /* omega in [0, 1]; 0.5 in the public implementation of the cited source [5] */
+    int   pcisph_min_iter, pcisph_max_iter;   /* sph_step_pcisph (reading R28): 0 => 3 / 100 */
 } SphParams;
 
 /* Rigid body = contiguous range of boundary samples (Akinci [3]).  Dynamics are
@@ -154,7 +161,9 @@ typedef enum SphField {
     SPH_FIELD_BOUNDARY_FORCE = 14, /* float [n_boundary*3] Eq. 14 reaction of the last step (dynamic samples only, else 0) */
     SPH_FIELD_RIGID_BODIES = 15,   /* SphRigidBody [n_bodies]                                rw */
     SPH_FIELD_BOUNDARY_CELL_START = 16, /* int [n_cells+1] boundary grid */
-    SPH_FIELD_BOUNDARY_CELL_OF_PARTICLE = 17 /* int [n_boundary] */
+    SPH_FIELD_BOUNDARY_CELL_OF_PARTICLE = 17, /* int [n_boundary] */
+    SPH_FIELD_KSUM_DIVERGENCE = 18,/* float [n_fluid]   total kappa^v_i the divergence solve applied in the last step (R27)  rw */
+    SPH_FIELD_KSUM_DENSITY = 19    /* float [n_fluid]   total kappa_i the density solve applied in the last step (R27)      rw */
 } SphField;
 
 typedef struct SphSim SphSim;

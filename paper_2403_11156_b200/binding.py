@@ -21,7 +21,7 @@ SPH_OK, SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA, SPH_EDOMAIN, SPH_ESTATE = 0, -1, -2, 
 # SphField
 (POS, VEL, DENSITY, ALPHA, KAPPA_OVER_RHO, CELL_START, CELL_OF_PARTICLE, SORTED_ID, NEIGHBOR_COUNT,
  FLUID_NEIGHBORS, BOUNDARY_NEIGHBORS, BOUNDARY_POS, BOUNDARY_VEL, BOUNDARY_PSI, BOUNDARY_FORCE,
- RIGID_BODIES, BOUNDARY_CELL_START, BOUNDARY_CELL_OF_PARTICLE) = range(18)
+ RIGID_BODIES, BOUNDARY_CELL_START, BOUNDARY_CELL_OF_PARTICLE, KSUM_DIVERGENCE, KSUM_DENSITY) = range(20)
 
 EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid", "sph_step_dfsph",
            "sph_step_wcsph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
@@ -44,6 +44,8 @@ class SphParams(C.Structure):
         ("max_fluid_neighbors", C.c_int), ("max_boundary_neighbors", C.c_int),
         ("use_cuda_graph", C.c_int), ("use_neighbor_list", C.c_int),
         ("cfl_factor", C.c_float), ("dt_min", C.c_float),
+        ("warm_start", C.c_int), ("warm_start_factor", C.c_float),
+        ("pcisph_min_iter", C.c_int), ("pcisph_max_iter", C.c_int),
     ]
 
 
@@ -123,7 +125,7 @@ def make_params(prm: Dict[str, object]) -> SphParams:
     """dict (keys of scenes.default_params + optional library switches) -> SphParams."""
     p = SphParams()
     defaults = dict(max_fluid_neighbors=0, max_boundary_neighbors=0, use_cuda_graph=1, use_neighbor_list=1,
-                    cfl_factor=0.0, dt_min=0.0)
+                    cfl_factor=0.0, dt_min=0.0, warm_start=0, warm_start_factor=0.5, pcisph_min_iter=0, pcisph_max_iter=0)
     for name, ctype in SphParams._fields_:
         val = prm.get(name, defaults.get(name))
         if val is None:
@@ -255,6 +257,7 @@ class Sim:
         table = {
             POS: ((nf, 3), t.float32), VEL: ((nf, 3), t.float32), DENSITY: ((nf,), t.float32),
             ALPHA: ((nf,), t.float32), KAPPA_OVER_RHO: ((nf,), t.float32),
+            KSUM_DIVERGENCE: ((nf,), t.float32), KSUM_DENSITY: ((nf,), t.float32),
             CELL_START: ((self.ncells + 1,), t.int32), CELL_OF_PARTICLE: ((nf,), t.int32),
             SORTED_ID: ((nf,), t.int32), NEIGHBOR_COUNT: ((nf, 2), t.int32),
             FLUID_NEIGHBORS: ((nf, self.kf), t.int32), BOUNDARY_NEIGHBORS: ((nf, self.kb), t.int32),

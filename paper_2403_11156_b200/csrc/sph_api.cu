@@ -58,6 +58,7 @@ struct SphSim {
     PV *pvB = nullptr, *pvC = nullptr;   // { pos | vel, rho } records of the passes; pvC: output of explicit viscosity
     int *idA = nullptr, *idB = nullptr;
     float *alpha = nullptr, *rho = nullptr;
+    float *ksum_v = nullptr, *ksum_d = nullptr;   // warm start: running totals of the step's solves (sorted order)
     GridBufs gf, gb;
     uint16_t *nl_f = nullptr;       // 16-bit (run, offset) entries, warp-tiled (sph_passes.cuh)
     int *nl_b = nullptr, *ncount = nullptr;
@@ -213,6 +214,9 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     c.visc_eps = (float)(0.01 * hd * hd);
     c.wc_k = p.wcsph_stiffness; c.wc_gamma = p.wcsph_exponent;
     c.has_dynamic = 0;
+    c.warm = p.warm_start ? 1 : 0;
+    c.warm_w = p.warm_start_factor;
+    if (p.warm_start && !(p.warm_start_factor >= 0.f && p.warm_start_factor <= 1.f)) { why = "warm_start_factor must lie in [0, 1]"; return false; }
     return true;
 }
 
@@ -235,6 +239,7 @@ size_t layout(SphSim &s, void *base)
     s.posk = w.take<float4>(nf1);
     s.alpha = w.take<float>(nf1);
     s.rho = w.take<float>(nf1);
+    if (s.prm.warm_start) { s.ksum_v = w.take<float>(nf1); s.ksum_d = w.take<float>(nf1); }
     s.gf.n = (int)nf;
     s.gf.key = w.take<int>(nf1); s.gf.off = w.take<int>(nf1); s.gf.slot = w.take<int>(nf1);
     s.gf.cell_start = w.take<int>(s.cs_len);
@@ -437,10 +442,11 @@ int run_loop(SphSim *s, bool graph_mode, long long *body_counter, Init init, Bod
 template <bool LIST>
 int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, PV *vel, int first)
 {
+    float *ksum = mode == MODE_DIV ? s->ksum_v : s->ksum_d;       // NULL unless warm start is on
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
     LoopHandle lh{ lc.h, lc.use_handle };
-#define SOLP(MODE, DYN) LAUNCH(s, (k_solver_p<LIST, MODE, DYN>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->ctl, s->stats, lh, first)
+#define SOLP(MODE, DYN) LAUNCH(s, (k_solver_p<LIST, MODE, DYN>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->ctl, s->stats, lh, first, ksum)
     if (mode == MODE_DIV) { if (dyn) SOLP(MODE_DIV, true); else SOLP(MODE_DIV, false); }
     else                  { if (dyn) SOLP(MODE_DENS, true); else SOLP(MODE_DENS, false); }
 #undef SOLP
@@ -449,7 +455,7 @@ int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, PV *vel, int first)
 
 // C-pass (with the tail work of the loop's last iteration) and the Eq. 14 reactions
 template <bool LIST>
-int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, PV *vel)
+int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, PV *vel, int force_mid = 0)
 {
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
@@ -459,6 +465,8 @@ int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, PV *vel)
     t.add_gravity = s->prm.viscosity_mode != 1;
     t.id = s->idB; t.pos_out = s->posA; t.vel_out = s->velA; t.id_out = s->idA;
     t.vmax_bits = &s->stats->vmax_bits; t.nan_count = &s->stats->nan_count;
+    t.force_mid = force_mid;
+    t.ksum_v = tail == TAIL_WCSPH ? nullptr : s->ksum_v; t.ksum_d = tail == TAIL_WCSPH ? nullptr : s->ksum_d;
     if (tail == TAIL_DIV)       LAUNCH(s, (k_solver_c<LIST, TAIL_DIV>), s->nblocks, kBlock, st, p, s->posk, vel, t);
     else if (tail == TAIL_DENS) LAUNCH(s, (k_solver_c<LIST, TAIL_DENS>), s->nblocks, kBlock, st, p, s->posk, vel, t);
     else                        LAUNCH(s, (k_solver_c<LIST, TAIL_WCSPH>), s->nblocks, kBlock, st, p, s->posk, vel, t);
@@ -499,8 +507,20 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
             // inside k_density_alpha (which also sets the predicate), the first C-pass follows,
             // further iterations (rare under the default tolerance) are the WHILE body.  The last
             // C-pass adds dt g (A6) unless a viscosity kernel follows.
+            const bool warm = s->c.warm != 0;
+            if (warm) {
+                // reading R27: rho, alpha alone (the fused first P-pass would see the velocities BEFORE the warm start),
+                // then the warm-start C-pass of the divergence solve; the loop's first P-pass is an ordinary launch
+                LoopCtx plain{ st, 0, 0 };
+                rc = enqueue_density(s, plain, false);
+                if (rc) return rc;
+                LAUNCH(s, k_warm_prepare<MODE_DIV>, cdiv(nf, 256), 256, st, s->c, s->posB, s->pvB, s->rho, s->ctl, s->posk, s->ksum_v);
+                rc = enqueue_solver_c<LIST>(s, st, TAIL_DIV, s->pvB, 1);
+                if (rc) return rc;
+            }
             rc = run_loop(s, graph_mode, &bc[LOOP_DIV],
                 [&](const LoopCtx &lc) -> int {
+                    if (warm) return enqueue_solver_iteration<LIST>(s, lc, MODE_DIV, s->pvB, 1);
                     int r = enqueue_density(s, lc, true);
                     if (r) return r;
                     return enqueue_solver_c<LIST>(s, lc.st, TAIL_DIV, s->pvB);
@@ -529,6 +549,11 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
                 if (rc) return rc;
             }
             // constant-density solve (A7), peeled the same way; its last C-pass integrates (A9)
+            if (warm) {
+                LAUNCH(s, k_warm_prepare<MODE_DENS>, cdiv(nf, 256), 256, st, s->c, s->posB, vcur, s->rho, s->ctl, s->posk, s->ksum_d);
+                rc = enqueue_solver_c<LIST>(s, st, TAIL_DENS, vcur, 1);
+                if (rc) return rc;
+            }
             rc = run_loop(s, graph_mode, &bc[LOOP_DENS],
                 [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur, 1); },
                 [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur, 0); });
@@ -621,6 +646,7 @@ bool field_info(const SphSim *s, int field, FieldInfo &fi)
     switch (field) {
     case SPH_FIELD_POS: case SPH_FIELD_VEL: fi = { nf * 12, true, false }; return true;
     case SPH_FIELD_DENSITY: case SPH_FIELD_ALPHA: case SPH_FIELD_KAPPA_OVER_RHO: fi = { nf * 4, false, true }; return true;
+    case SPH_FIELD_KSUM_DIVERGENCE: case SPH_FIELD_KSUM_DENSITY: fi = { nf * 4, true, false }; return true;
     case SPH_FIELD_CELL_START: fi = { nc1 * 4, false, true }; return true;
     case SPH_FIELD_CELL_OF_PARTICLE: case SPH_FIELD_SORTED_ID: fi = { nf * 4, false, true }; return true;
     case SPH_FIELD_NEIGHBOR_COUNT: fi = { nf * 8, false, true }; return true;
@@ -645,6 +671,8 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
     switch (field) {
     case SPH_FIELD_POS: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->posA, s->idA, nf, (float *)out); break;
     case SPH_FIELD_VEL: LAUNCH(s, k_export_vec3, cdiv(nf, 256), 256, st, s->velA, s->idA, nf, (float *)out); break;
+    case SPH_FIELD_KSUM_DIVERGENCE: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->velA, s->idA, nf, (float *)out, 1); break;
+    case SPH_FIELD_KSUM_DENSITY: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posA, s->idA, nf, (float *)out, 1); break;
     case SPH_FIELD_DENSITY: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->rho, s->idB, nf, (float *)out); break;
     case SPH_FIELD_ALPHA: LAUNCH(s, k_export_scalar, cdiv(nf, 256), 256, st, s->alpha, s->idB, nf, (float *)out); break;
     case SPH_FIELD_KAPPA_OVER_RHO: LAUNCH(s, k_export_w, cdiv(nf, 256), 256, st, s->posk, s->idB, nf, (float *)out, 1); break;
@@ -682,6 +710,8 @@ int import_field(SphSim *s, int field, const void *src, size_t bytes)
     switch (field) {
     case SPH_FIELD_POS: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->posA); break;
     case SPH_FIELD_VEL: LAUNCH(s, k_import_vec3, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->velA); s->vmax_valid = false; break;
+    case SPH_FIELD_KSUM_DIVERGENCE: LAUNCH(s, k_import_w, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->velA); break;
+    case SPH_FIELD_KSUM_DENSITY: LAUNCH(s, k_import_w, cdiv(nf, 256), 256, st, (const float *)src, s->idA, nf, s->posA); break;
     case SPH_FIELD_BOUNDARY_POS: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_pos); s->boundary_dirty |= DIRTY_BPOS; break;
     case SPH_FIELD_BOUNDARY_VEL: LAUNCH(s, k_import_vec3, cdiv(nb, 256), 256, st, (const float *)src, (const int *)nullptr, nb, s->borig_vel); s->boundary_dirty |= DIRTY_BVEL; break;
     case SPH_FIELD_RIGID_BODIES:

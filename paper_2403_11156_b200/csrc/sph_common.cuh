@@ -48,6 +48,8 @@ struct SimConst {
     float visc_eps;      // 0.01 h^2                (Eq. 15 / 19, R4)
     float wc_k, wc_gamma;
     int has_dynamic;     // any dynamic rigid body
+    int warm;            // warm start of both DFSPH solves (reading R27)
+    float warm_w;        // omega
 };
 
 // Loop-control block in device memory (one per simulation).  Written by the host only through

@@ -422,7 +422,7 @@ template <bool LIST, int MODE, bool DYN>
 __global__ void __launch_bounds__(kBlock)
 k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel,
            const float *__restrict__ alpha, float4 *__restrict__ posk,
-           DevControl *ctl, DevStats *st, LoopHandle lh, int first)
+           DevControl *ctl, DevStats *st, LoopHandle lh, int first, float *__restrict__ ksum)
 {
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
@@ -453,6 +453,8 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
         if (MODE == MODE_DIV) {
             term = fmaxf(D, 0.f);
             kappa = a * term / dt;
+            // (warm-start path only: there this launch opens the divergence loop, which may be switched off)
+            if (first && !(ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0)) kappa = 0.f;
         } else {
             term = fmaxf(fmaf(dt, D, rho), c.rho0) - c.rho0;
             kappa = a * term / (dt * dt);
@@ -461,8 +463,30 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
             if (first && !(ctl->forced_d != 0 && ctl->max_d > 0)) kappa = 0.f;
         }
         posk[i] = make_float4(xi.x, xi.y, xi.z, kappa / rho);
+        if (ksum != nullptr) ksum[i] += kappa;                     // running total of the solve (warm start, R27)
     }
     solver_tail<MODE>(c, term, ctl, st, lh, first != 0);
+}
+
+// Warm start (reading R27): before a solve's loop the total stiffness K_i that the
+// same solve applied in the LAST step, scaled by omega, is applied once through an ordinary C-pass with the
+// densities and gradients of the current step.  K_i travels with the particle in the fourth lane of the persistent
+// position (density solve) / velocity (divergence solve) and has been permuted by the sort.  This kernel writes
+// posk[i] = (x_i, omega K_i / rho_i) and starts the solve's running total at omega K_i (0 when the solve is off).
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_warm_prepare(SimConst c, const float4 *__restrict__ pos, const PV *__restrict__ pv, const float *__restrict__ rho,
+               const DevControl *__restrict__ ctl, float4 *__restrict__ posk, float *__restrict__ ksum)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.nf) return;
+    const bool on = MODE == MODE_DIV ? (ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0)
+                                     : (ctl->forced_d != 0 && ctl->max_d > 0);
+    const float4 x = pos[i];
+    const float K = MODE == MODE_DIV ? pv[i].v.w : x.w;
+    const float k = on ? c.warm_w * K : 0.f;
+    posk[i] = make_float4(x.x, x.y, x.z, k / rho[i]);
+    ksum[i] = k;
 }
 
 // C-pass (A5 / A7 / A10): pressure-like velocity update (Eq. 7 + Eq. 13 with p/rho^2 == kappa/rho,
@@ -485,6 +509,8 @@ struct CTail {
     int *id_out;
     unsigned *vmax_bits;
     int *nan_count;
+    int force_mid;            // 1: this launch is never the loop's last one (the warm-start C-pass, reading R27)
+    const float *ksum_v, *ksum_d;   // warm start: totals of this step's solves, stored with the persistent state (else NULL)
 };
 
 template <bool LIST, int TAIL>
@@ -494,7 +520,7 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, PV *__restrict__ pv, CTai
     __shared__ int tbl[LIST ? kRows * kBlock : 1];
     const SimConst &c = p.c;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool last = TAIL == TAIL_WCSPH || t.ctl->cont == 0;
+    const bool last = !t.force_mid && (TAIL == TAIL_WCSPH || t.ctl->cont == 0);
     float v2 = 0.f;
     bool bad = false;
     if (i < c.nf) {
@@ -530,9 +556,10 @@ k_solver_c(PassCtx p, const float4 *__restrict__ posk, PV *__restrict__ pv, CTai
             if (last) {
                 float4 x;
                 x.x = fmaf(dt, v.x, xi.x); x.y = fmaf(dt, v.y, xi.y); x.z = fmaf(dt, v.z, xi.z);
-                x.w = 0.f;
+                // the fourth lanes of the persistent store carry the warm-start totals through the next sort (R27)
+                x.w = t.ksum_d != nullptr ? t.ksum_d[i] : 0.f;
                 t.pos_out[i] = x;
-                t.vel_out[i] = make_float4(v.x, v.y, v.z, 0.f);
+                t.vel_out[i] = make_float4(v.x, v.y, v.z, t.ksum_v != nullptr ? t.ksum_v[i] : 0.f);
                 t.id_out[i] = t.id[i];
                 v2 = fmaf(v.x, v.x, fmaf(v.y, v.y, v.z * v.z));
                 bad = !(isfinite(x.x) && isfinite(x.y) && isfinite(x.z) && isfinite(v2));

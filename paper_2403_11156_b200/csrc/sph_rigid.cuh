@@ -56,6 +56,14 @@ k_import_vec3(const float *__restrict__ src, const int *__restrict__ id, int n, 
     v.x = src[3 * o]; v.y = src[3 * o + 1]; v.z = src[3 * o + 2];
     dst[s] = v;
 }
+// caller-order float[n] -> fourth lane of the sorted float4: dst[s].w = src[id[s]]
+__global__ void __launch_bounds__(256)
+k_import_w(const float *__restrict__ src, const int *__restrict__ id, int n, float4 *__restrict__ dst)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    dst[s].w = src[id[s]];
+}
 __global__ void __launch_bounds__(256)
 k_export_counts(const int *__restrict__ ncount, const int *__restrict__ id, int n, int *__restrict__ out)
 {

@@ -87,13 +87,17 @@ def sync_oracle_to_gpu(g, o, scene):
     """Copy the GPU's fp32 state (fluid, boundary samples, bodies) into the oracle."""
     from paper_2403_11156_b200 import binding as B
     o.set_state(np_(g.sph_read_state(B.POS)), np_(g.sph_read_state(B.VEL)))
+    if scene.params.get("warm_start", 0):
+        # the warm-start totals of the last step travel with the particles (reading R27)
+        o.set_warm_state(np_(g.sph_read_state(B.KSUM_DIVERGENCE)).astype(np.float64),
+                         np_(g.sph_read_state(B.KSUM_DENSITY)).astype(np.float64))
     if g.nb and any(b.dynamic for b in scene.bodies):
         o.set_boundary_state(np_(g.sph_read_state(B.BOUNDARY_POS)), np_(g.sph_read_state(B.BOUNDARY_VEL)))
         from paper_2403_11156_b200.scenes import Body
         o.set_bodies([Body(**b) for b in g.read_bodies()])
 
 
-def resync_step(g, o, scene, method="dfsph"):
+def resync_step(g, o, scene, method="dfsph", dv_floor_per_pass=None):
     """One step on both from the GPU's current state, the oracle forced to the GPU's iteration
     counts (several counts are valid when err ~ eta: reading R20).  Returns (errors, gpu stats)."""
     sync_oracle_to_gpu(g, o, scene)
@@ -117,5 +121,7 @@ def resync_step(g, o, scene, method="dfsph"):
     # the floor sqrt(|g| H) of the velocity norm hides nothing large: relative to the ACTUAL
     # velocity scale the error is 1e-4 plus the absolute noise floor fp32 leaves through rho* - rho0
     # (~2e-5 m/s), so a regression in the slow-flow regime is caught as well
-    assert e["dv_abs"] <= 1e-4 * e["vscale_raw"] + 5e-5, e
+    # dv_floor_per_pass: steps with many solver iterations (tight tolerance) accumulate that floor once per C-pass
+    floor = 5e-5 if dv_floor_per_pass is None else dv_floor_per_pass * max(2, st["it_v"] + st["it_d"] + 2)
+    assert e["dv_abs"] <= 1e-4 * e["vscale_raw"] + floor, (e, floor)
     return e, st

@@ -8,6 +8,7 @@ v: max|dv| / max(max|v|, sqrt(|g| H)).  Positions follow from v: |dx| <= dt * to
 """
 import numpy as np
 import pytest
+import torch
 
 from paper_2403_11156_b200 import scenes
 
@@ -708,3 +709,40 @@ def test_cfl_adaptive_time_step_parity(B, oracle):
         outs.append((gg.sph_read_state(B.POS).clone(), gg.sph_read_stats()["sim_time"]))
         gg.close()
     assert torch.equal(outs[0][0], outs[1][0]) and outs[0][1] == outs[1][1]
+
+
+# ------------------------------------------------------------------ NEXT-1: warm start (reading R27)
+
+def test_warm_start_parity_and_fewer_iterations(B, oracle):
+    """Hydrostatic column under a tight tolerance (the oracle pin's scene): the warm-started CUDA step matches the
+    warm-started oracle step from the same state AND the same stored totals (rho, alpha, v, x within 1e-4; the new
+    totals within 1e-4 of their maximum), the totals survive the sort and a write/read round trip, and the
+    warm-started run needs clearly fewer density iterations than the cold one."""
+    kw = dict(dt=1e-3, eta_density=1e-4, min_iter_density=1)
+    sc = scenes.dam_break((8, 8, 30), (8, 8, 34), warm_start=1, warm_start_factor=0.5, **kw)
+    g, o = make_pair(sc, oracle)
+    g.sph_step_dfsph(45)
+    for _ in range(3):
+        e, st = resync_step(g, o, sc, dv_floor_per_pass=2.5e-5)    # ~10 C-passes per step here
+        check_errors(e, sc)
+        assert st["it_d"] >= 1 and st["err_rho"] <= 1e-4
+        for fld, ref in ((B.KSUM_DENSITY, o.ksum_d()), (B.KSUM_DIVERGENCE, o.ksum_v())):
+            got = np_(g.sph_read_state(fld)).astype(np.float64)
+            assert np.abs(got - ref).max() <= 1e-4 * max(np.abs(ref).max(), 1e-30)
+        assert o.ksum_d().max() > 0.0
+        g.sph_step_dfsph(4)
+    warm_total = g.sph_read_stats()["total_it_d"]
+    # round trip of the totals through the ABI (id order, un-permuted)
+    kd = g.sph_read_state(B.KSUM_DENSITY).clone()
+    g.sph_write_state(B.KSUM_DENSITY, kd * 0.5)
+    assert torch.equal(g.sph_read_state(B.KSUM_DENSITY), kd * 0.5)
+    steps = g.sph_read_stats()["steps_done"]
+    g.close(); o.close()
+    cold = B.Sim.from_scene(scenes.dam_break((8, 8, 30), (8, 8, 34), **kw))
+    cold.sph_step_dfsph(int(steps))
+    st = cold.sph_read_stats()
+    assert st["err_rho"] <= 1e-4
+    assert warm_total <= 0.75 * st["total_it_d"], (warm_total, st["total_it_d"])
+    # totals are zero without warm start
+    assert float(cold.sph_read_state(B.KSUM_DENSITY).abs().max()) == 0.0
+    cold.close()
