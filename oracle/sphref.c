@@ -580,6 +580,71 @@ int sphref_density_solve(SphRef *s, double *vel, int forced)
     return l;
 }
 
+/* ------------------------------------------------------------------ PCISPH (reading R28) */
+
+/* PCISPH scaling factor of the cited source [25] (PAPER.md:158, 264 name the method; the paper prints none of its
+ * equations -- reading R28):  delta = 1 / (beta (|sum_j gradW_ij|^2 + sum_j |gradW_ij|^2)),  beta = 2 (dt m / rho0)^2,
+ * evaluated ONCE for a prototype particle with a filled neighbourhood: the sites of a simple-cubic lattice of spacing 2r
+ * strictly inside the support radius h (the first sum vanishes there by symmetry, it is kept for the definition's sake).
+ * Returned WITHOUT the dt^-2 factor:  k = rho0^2 / (2 m^2 (...)),  delta = k / dt^2  (dt may change per step, R26). */
+double sphref_pcisph_k(const SphRef *s)
+{
+    double h = s->p.support_radius, sp = 2.0 * s->p.particle_radius, m = s->m;
+    int n = (int)ceil(h / sp) + 1;
+    double S[3] = { 0, 0, 0 }, T = 0.0, g[3];
+    for (int a = -n; a <= n; ++a) for (int b = -n; b <= n; ++b) for (int c = -n; c <= n; ++c) {
+        if (a == 0 && b == 0 && c == 0) continue;
+        double d[3] = { -a * sp, -b * sp, -c * sp };            /* x_i - x_j, particle i at the origin */
+        if (dot3(d, d) >= h * h) continue;
+        sphref_gradW(d, h, g);
+        for (int q = 0; q < 3; ++q) S[q] += g[q];
+        T += dot3(g, g);
+    }
+    return s->p.rest_density * s->p.rest_density / (2.0 * m * m * (dot3(S, S) + T));
+}
+
+/* PCISPH pressure loop in the form of Alg. 2 with the density-based source term, Eq. 8, and the
+ * prediction of Eq. 9: starting from p = 0 and the velocities v* after the non-pressure forces,
+ *   do { P: rho*_i = rho_i + dt D_i[v*]                                (Eq. 9 times ... with D of (c.1))
+ *           err = mean_i max(rho*_i - rho0, 0) / rho0                   (same measure as the DFSPH density solve, R6)
+ *           p_i(new) = max(p_i + delta (rho*_i - rho0), 0)              ([25]: global delta, pressure clamped at zero)
+ *        C: v* <- v* - dt U[(p_i(new) - p_i) / rho_i^2]                 (Eq. 7 + 13; the pressure force is linear in p,
+ *                                                                        so applying the increment equals recomputing
+ *                                                                        the force from the accumulated pressure)
+ *           l++ }
+ * while ((err > eta_density || l < pcisph_min_iter) && l < pcisph_max_iter)   ([25] asks for at least 3 iterations).
+ * forced >= 0: exactly that many iterations.  s->kappa holds the accumulated pressure on return. */
+int sphref_pcisph_solve(SphRef *s, double *vel, int forced)
+{
+    const SphRefParams *p = &s->p;
+    int l = 0;
+    double err = 0.0;
+    double delta = sphref_pcisph_k(s) / (p->dt * p->dt);
+    int mn = p->pcisph_min_iter > 0 ? p->pcisph_min_iter : 3, mx = p->pcisph_max_iter > 0 ? p->pcisph_max_iter : 100;
+    for (int i = 0; i < s->nf; ++i) s->kappa[i] = 0.0;
+    if (forced == 0) { s->stats.it_d = 0; s->stats.err_rho = 0.0; return 0; }
+    for (;;) {
+        double sum = 0.0;
+#pragma omp parallel for schedule(dynamic, 256) reduction(+ : sum)
+        for (int i = 0; i < s->nf; ++i) {
+            double rs = s->rho[i] + p->dt * density_rate(s, vel, i);
+            double e = rs - p->rest_density;
+            sum += e > 0.0 ? e : 0.0;
+            double pn = s->kappa[i] + delta * e;
+            if (pn < 0.0) pn = 0.0;
+            s->kr[i] = (pn - s->kappa[i]) / (s->rho[i] * s->rho[i]);
+            s->kappa[i] = pn;
+        }
+        err = s->nf > 0 ? sum / s->nf / p->rest_density : 0.0;
+        apply_pressure_update(s, vel);
+        ++l;
+        if (forced > 0) { if (l >= forced) break; }
+        else if (!((err > p->eta_density || l < mn) && l < mx)) break;
+    }
+    s->stats.it_d = l; s->stats.err_rho = err;
+    return l;
+}
+
 /* ------------------------------------------------------------------ viscosity */
 
 /* Shared pair factor of Eq. 15 / Eq. 19: (v_ij . x_ij) / (|x_ij|^2 + 0.01 h^2) gradW_ij
@@ -829,6 +894,36 @@ int sphref_step_wcsph(SphRef *s)
     s->stats.dt_last = s->p.dt; s->stats.sim_time += s->p.dt;
     s->p.dt = s->dt_max;
     free(rt); free(acc);
+    s->lists_valid = 0;
+    return 0;
+}
+
+/* One PCISPH step (reading R28; Alg. 1 PAPER.md:127-134 with the pressure solve of Alg. 2 realised by [25]):
+ * grid -> rho (Eq. 12) -> v* = v + dt (g + Eq. 15 if viscosity_mode 1) -> pressure loop above -> x += dt v* -> rigid step.
+ * (viscosity_mode 2 is not combined with this solver.) */
+int sphref_step_pcisph(SphRef *s, int forced)
+{
+    const SphRefParams *p = &s->p;
+    int n3 = 3 * s->nf;
+    s->p.dt = choose_dt(s);
+    if (p->force_iterations && forced < 0) forced = p->pcisph_min_iter > 0 ? p->pcisph_min_iter : 3;
+    sphref_build_grid(s);
+    memset(s->bforce, 0, sizeof(double) * 3 * (size_t)(s->nb > 0 ? s->nb : 1));
+    sphref_compute_density_alpha(s);
+    if (p->viscosity_mode == 1) {
+        double *acc = (double *)malloc(sizeof(double) * (size_t)(n3 + 1));
+        sphref_explicit_viscosity_accel(s, s->v, s->rho, acc);
+        for (int i = 0; i < n3; ++i) s->v[i] += p->dt * (p->gravity[i % 3] + acc[i]);
+        free(acc);
+    } else {
+        for (int i = 0; i < n3; ++i) s->v[i] += p->dt * p->gravity[i % 3];
+    }
+    sphref_pcisph_solve(s, s->v, forced);
+    for (int i = 0; i < n3; ++i) s->x[i] += p->dt * s->v[i];
+    sphref_rigid_step(s);
+    s->stats.it_v = 0; s->stats.cg_iters = 0; s->stats.v_max = max_speed(s);
+    s->stats.dt_last = s->p.dt; s->stats.sim_time += s->p.dt;
+    s->p.dt = s->dt_max;
     s->lists_valid = 0;
     return 0;
 }

@@ -88,6 +88,10 @@ def lib():
         L.sphref_step_dfsph.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.sphref_divergence_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.sphref_density_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.sphref_pcisph_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.sphref_step_pcisph.argtypes = [C.c_void_p, C.c_int]
+        L.sphref_pcisph_k.argtypes = [C.c_void_p]
+        L.sphref_pcisph_k.restype = C.c_double
         L.sphref_implicit_viscosity_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.sphref_explicit_viscosity_accel.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sphref_viscosity_operator.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -237,6 +241,17 @@ class Sim:
 
     def density_solve(self, vel, forced: int = -1):
         return self._solve(lib().sphref_density_solve, vel, forced)
+
+    def pcisph_solve(self, vel, forced: int = -1):
+        """PCISPH pressure loop (reading R28) on the given velocities; accumulated pressure in kappa()."""
+        return self._solve(lib().sphref_pcisph_solve, vel, forced)
+
+    def step_pcisph(self, forced: int = -1):
+        lib().sphref_step_pcisph(self._h, forced)
+
+    def pcisph_k(self) -> float:
+        """delta dt^2 of reading R28 (prototype-lattice constant)."""
+        return float(lib().sphref_pcisph_k(self._h))
 
     def implicit_viscosity_solve(self, vel, forced: int = -1):
         return self._solve(lib().sphref_implicit_viscosity_solve, vel, forced)
