@@ -199,6 +199,15 @@ int sph_step_dfsph(SphSim *sim, int n_steps);
 /* n_steps WCSPH steps (PAPER.md:140 EOS; Eq. 7, 12, 13; R17): fixed work per step. */
 int sph_step_wcsph(SphSim *sim, int n_steps);
 
+/* n_steps PCISPH steps (the paper's second PPE solver; cited source [25]; reading R28):
+ * grid -> rho -> v* = v + dt (g [+ Eq. 15]) -> pressure loop of Alg. 2 with the density source term (Eq. 8) and the
+ * prediction of Eq. 9: p_i <- max(p_i + delta (rho*_i - rho0), 0) with the global scaling factor delta of [25]
+ * (prototype particle in a filled lattice neighbourhood), the increment applied through Eq. 7 + 13; at least
+ * pcisph_min_iter iterations, until mean(max(rho* - rho0, 0)) / rho0 <= eta_density -> symplectic Euler -> rigid
+ * bodies.  SphStats.it_d / err_rho report the loop; forced_d of sph_set_forced_iterations overrides its count.
+ * viscosity_mode 2 is not combined with this solver (SPH_ESTATE). */
+int sph_step_pcisph(SphSim *sim, int n_steps);
+
 /* Override the iteration counts of the next steps: -1 = tolerances decide, >= 0 = exactly that
  * many iterations of the divergence solve / density solve / CG.  Takes effect without re-capture.
  * Synchronises the stream. */

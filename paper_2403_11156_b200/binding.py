@@ -24,7 +24,7 @@ SPH_OK, SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA, SPH_EDOMAIN, SPH_ESTATE = 0, -1, -2, 
  RIGID_BODIES, BOUNDARY_CELL_START, BOUNDARY_CELL_OF_PARTICLE, KSUM_DIVERGENCE, KSUM_DENSITY) = range(20)
 
 EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid", "sph_step_dfsph",
-           "sph_step_wcsph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
+           "sph_step_wcsph", "sph_step_pcisph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
            "sph_read_stats", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
            "sph_last_error", "sph_destroy"]
 
@@ -105,6 +105,7 @@ def load() -> C.CDLL:
         L.sph_build_grid.argtypes = [C.c_void_p]
         L.sph_step_dfsph.argtypes = [C.c_void_p, C.c_int]
         L.sph_step_wcsph.argtypes = [C.c_void_p, C.c_int]
+        L.sph_step_pcisph.argtypes = [C.c_void_p, C.c_int]
         L.sph_set_forced_iterations.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.sph_read_state.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_int]
         L.sph_write_state.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_int]
@@ -247,6 +248,9 @@ class Sim:
 
     def sph_step_wcsph(self, n_steps: int = 1):
         self._check(load().sph_step_wcsph(self._h, n_steps))
+
+    def sph_step_pcisph(self, n_steps: int = 1):
+        self._check(load().sph_step_pcisph(self._h, n_steps))
 
     def sph_set_forced_iterations(self, forced_v: int = -1, forced_d: int = -1, forced_cg: int = -1):
         self._check(load().sph_set_forced_iterations(self._h, forced_v, forced_d, forced_cg))

@@ -59,6 +59,7 @@ struct SphSim {
     int *idA = nullptr, *idB = nullptr;
     float *alpha = nullptr, *rho = nullptr;
     float *ksum_v = nullptr, *ksum_d = nullptr;   // warm start: running totals of the step's solves (sorted order)
+    float *pacc = nullptr;          // PCISPH: accumulated pressure of the running step (sorted order)
     GridBufs gf, gb;
     uint16_t *nl_f = nullptr;       // 16-bit (run, offset) entries, warp-tiled (sph_passes.cuh)
     int *nl_b = nullptr, *ncount = nullptr;
@@ -77,12 +78,13 @@ struct SphSim {
     // host
     int *pinned = nullptr;          // small pinned block (loop predicate, stats)
     int boundary_dirty = 0;         // DIRTY_* bits: boundary fields written through sph_write_state since the last refresh
+    bool pci_step = false;          // the step being enqueued is a PCISPH step
     bool vmax_valid = false;        // stats->vmax_bits = max |v| of the persistent store (needed by the CFL rule)
     bool derived_valid = false;     // B-order fields (rho, alpha, lists, cell_start) match the store
-    cudaGraphExec_t exec[2] = { nullptr, nullptr };   // 0 DFSPH, 1 WCSPH
-    long long fixed_nodes[2] = { 0, 0 };
-    long long body_nodes[2][3] = { { 0, 0, 0 }, { 0, 0, 0 } };
-    long long graph_steps[2] = { 0, 0 };              // graph launches per method (host view)
+    cudaGraphExec_t exec[3] = { nullptr, nullptr, nullptr };   // 0 DFSPH, 1 WCSPH, 2 PCISPH
+    long long fixed_nodes[3] = { 0, 0, 0 };
+    long long body_nodes[3][3] = { { 0, 0, 0 }, { 0, 0, 0 }, { 0, 0, 0 } };
+    long long graph_steps[3] = { 0, 0, 0 };           // graph launches per method (host view)
     long long misc_launches = 0;
     long long *cur_counter = nullptr;
     // optional per-kernel CUDA-event timing (host-driven launch mode only, see sph_enable_kernel_timing)
@@ -213,6 +215,25 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     c.mu = p.kinematic_viscosity * p.rest_density;      // R21
     c.visc_eps = (float)(0.01 * hd * hd);
     c.wc_k = p.wcsph_stiffness; c.wc_gamma = p.wcsph_exponent;
+    {
+        // PCISPH scaling factor (reading R28, cited source [25]): delta dt^2 = rho0^2 / (2 m^2 (|sum gradW|^2 + sum |gradW|^2))
+        // for a prototype particle inside a simple-cubic lattice of spacing 2r, neighbours strictly inside h
+        const double sp = d, h = hd;
+        const int n = (int)std::ceil(h / sp) + 1;
+        double S[3] = { 0, 0, 0 }, T = 0.0;
+        for (int ia = -n; ia <= n; ++ia) for (int ib = -n; ib <= n; ++ib) for (int ic = -n; ic <= n; ++ic) {
+            if (!ia && !ib && !ic) continue;
+            const double dx = -ia * sp, dy = -ib * sp, dz = -ic * sp, r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 >= h * h) continue;
+            const double r = std::sqrt(r2), q = r / h;
+            const double wp = q <= 0.5 ? 6.0 * q * (3.0 * q - 2.0) : -6.0 * (1.0 - q) * (1.0 - q);
+            const double f = sigma / h * wp / r;
+            S[0] += f * dx; S[1] += f * dy; S[2] += f * dz;
+            T += f * f * r2;
+        }
+        const double den = 2.0 * (double)c.m * (double)c.m * (S[0] * S[0] + S[1] * S[1] + S[2] * S[2] + T);
+        c.pci_k = den > 0.0 ? (float)((double)p.rest_density * (double)p.rest_density / den) : 0.f;
+    }
     c.has_dynamic = 0;
     c.warm = p.warm_start ? 1 : 0;
     c.warm_w = p.warm_start_factor;
@@ -240,6 +261,7 @@ size_t layout(SphSim &s, void *base)
     s.alpha = w.take<float>(nf1);
     s.rho = w.take<float>(nf1);
     if (s.prm.warm_start) { s.ksum_v = w.take<float>(nf1); s.ksum_d = w.take<float>(nf1); }
+    s.pacc = w.take<float>(nf1);
     s.gf.n = (int)nf;
     s.gf.key = w.take<int>(nf1); s.gf.off = w.take<int>(nf1); s.gf.slot = w.take<int>(nf1);
     s.gf.cell_start = w.take<int>(s.cs_len);
@@ -442,12 +464,13 @@ int run_loop(SphSim *s, bool graph_mode, long long *body_counter, Init init, Bod
 template <bool LIST>
 int enqueue_solver_p(SphSim *s, const LoopCtx &lc, int mode, PV *vel, int first)
 {
-    float *ksum = mode == MODE_DIV ? s->ksum_v : s->ksum_d;       // NULL unless warm start is on
+    float *ksum = mode == MODE_PCI ? s->pacc : (mode == MODE_DIV ? s->ksum_v : s->ksum_d);   // warm start totals (NULL when off) / PCISPH pressure
     PassCtx p = make_ctx(s);
     const bool dyn = s->c.has_dynamic != 0;
     LoopHandle lh{ lc.h, lc.use_handle };
 #define SOLP(MODE, DYN) LAUNCH(s, (k_solver_p<LIST, MODE, DYN>), s->nblocks, kBlock, lc.st, p, vel, s->bvel_s, s->alpha, s->posk, s->ctl, s->stats, lh, first, ksum)
     if (mode == MODE_DIV) { if (dyn) SOLP(MODE_DIV, true); else SOLP(MODE_DIV, false); }
+    else if (mode == MODE_PCI) { if (dyn) SOLP(MODE_PCI, true); else SOLP(MODE_PCI, false); }
     else                  { if (dyn) SOLP(MODE_DENS, true); else SOLP(MODE_DENS, false); }
 #undef SOLP
     return SPH_OK;
@@ -466,7 +489,8 @@ int enqueue_solver_c(SphSim *s, cudaStream_t st, int tail, PV *vel, int force_mi
     t.id = s->idB; t.pos_out = s->posA; t.vel_out = s->velA; t.id_out = s->idA;
     t.vmax_bits = &s->stats->vmax_bits; t.nan_count = &s->stats->nan_count;
     t.force_mid = force_mid;
-    t.ksum_v = tail == TAIL_WCSPH ? nullptr : s->ksum_v; t.ksum_d = tail == TAIL_WCSPH ? nullptr : s->ksum_d;
+    const bool keep_totals = tail != TAIL_WCSPH && !s->pci_step;   // only DFSPH steps maintain the warm-start totals
+    t.ksum_v = keep_totals ? s->ksum_v : nullptr; t.ksum_d = keep_totals ? s->ksum_d : nullptr;
     if (tail == TAIL_DIV)       LAUNCH(s, (k_solver_c<LIST, TAIL_DIV>), s->nblocks, kBlock, st, p, s->posk, vel, t);
     else if (tail == TAIL_DENS) LAUNCH(s, (k_solver_c<LIST, TAIL_DENS>), s->nblocks, kBlock, st, p, s->posk, vel, t);
     else                        LAUNCH(s, (k_solver_c<LIST, TAIL_WCSPH>), s->nblocks, kBlock, st, p, s->posk, vel, t);
@@ -481,7 +505,7 @@ int enqueue_solver_iteration(SphSim *s, const LoopCtx &lc, int mode, PV *vel, in
 {
     int rc = enqueue_solver_p<LIST>(s, lc, mode, vel, first);
     if (rc) return rc;
-    return enqueue_solver_c<LIST>(s, lc.st, mode == MODE_DIV ? TAIL_DIV : TAIL_DENS, vel);
+    return enqueue_solver_c<LIST>(s, lc.st, mode == MODE_DIV ? TAIL_DIV : TAIL_DENS, vel);   // MODE_PCI: the density loop's tail
 }
 
 template <bool LIST>
@@ -558,6 +582,23 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
                 [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur, 1); },
                 [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_DENS, vcur, 0); });
             if (rc) return rc;
+        } else if (method == 2) {
+            // PCISPH (reading R28): rho -> v* = v + dt (g [+ Eq. 15]) -> pressure loop (P-pass with the global delta,
+            // ordinary C-pass; peeled like the density loop, the last C-pass integrates) -> rigid bodies
+            LoopCtx plain{ st, 0, 0 };
+            rc = enqueue_density(s, plain, false);
+            if (rc) return rc;
+            LAUNCH(s, k_pci_begin, cdiv(nf, 256), 256, st, s->c, s->rho, s->pvB, s->pacc, s->prm.viscosity_mode != 1);
+            if (s->prm.viscosity_mode == 1) {
+                LAUNCH(s, (k_explicit_viscosity<LIST, false>), s->nblocks, kBlock, st, p, s->pvB, s->pvC);
+                vcur = s->pvC;
+            }
+            s->pci_step = true;
+            rc = run_loop(s, graph_mode, &bc[LOOP_DENS],
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_PCI, vcur, 1); },
+                [&](const LoopCtx &lc) -> int { return enqueue_solver_iteration<LIST>(s, lc, MODE_PCI, vcur, 0); });
+            s->pci_step = false;
+            if (rc) return rc;
         } else {
             // WCSPH (A10): rho, EOS, [viscosity], one C-pass that also adds dt g and integrates
             LoopCtx plain{ st, 0, 0 };
@@ -612,6 +653,7 @@ int do_steps(SphSim *s, int method, int n_steps)
 {
     if (!s) return SPH_EINVAL;
     if (n_steps < 0) { s->err = "n_steps < 0"; return SPH_EINVAL; }
+    if (method == 2 && s->prm.viscosity_mode == 2) { s->err = "sph_step_pcisph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
     if (method == 1 && s->prm.viscosity_mode == 2) { s->err = "sph_step_wcsph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
     DeviceGuard dg(s->device);
     if (n_steps > 0) { int rc = refresh_boundary(s); if (rc) return rc; }
@@ -817,11 +859,12 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
         memset(&hc, 0, sizeof hc);
         const SphParams &p = s->prm;
         hc.forced_v = p.force_iterations ? p.min_iter_divergence : -1;
-        hc.forced_d = p.force_iterations ? p.min_iter_density : -1;
+        hc.forced_d = p.force_iterations ? p.min_iter_density : -1;   // (PCISPH steps with force_iterations: set the count with sph_set_forced_iterations)
         hc.forced_cg = -1;
         hc.min_v = p.min_iter_divergence; hc.max_v = p.max_iter_divergence;
         hc.min_d = p.min_iter_density; hc.max_d = p.max_iter_density;
         hc.max_cg = p.cg_max_iter; hc.enable_div = p.enable_divergence_solve;
+        hc.min_p = p.pcisph_min_iter > 0 ? p.pcisph_min_iter : 3; hc.max_p = p.pcisph_max_iter > 0 ? p.pcisph_max_iter : 100;
         hc.dt = p.dt;
         hc.eta_v = p.eta_divergence; hc.eta_d = p.eta_density; hc.cg_tol = p.cg_rel_tol;
         memcpy(s->pinned, &hc, sizeof hc);
@@ -892,6 +935,7 @@ int sph_build_grid(SphSim *s)
 
 int sph_step_dfsph(SphSim *s, int n_steps) { return do_steps(s, 0, n_steps); }
 int sph_step_wcsph(SphSim *s, int n_steps) { return do_steps(s, 1, n_steps); }
+int sph_step_pcisph(SphSim *s, int n_steps) { return do_steps(s, 2, n_steps); }
 
 int sph_set_forced_iterations(SphSim *s, int forced_v, int forced_d, int forced_cg)
 {
@@ -973,15 +1017,15 @@ long long sph_launch_count(SphSim *s)
 {
     if (!s) return 0;
     long long n = s->misc_launches;
-    if (s->prm.use_cuda_graph && (s->graph_steps[0] + s->graph_steps[1]) > 0) {
+    if (s->prm.use_cuda_graph && (s->graph_steps[0] + s->graph_steps[1] + s->graph_steps[2]) > 0) {
         SphStats st;
         if (sph_read_stats(s, &st) != SPH_OK) return n;
         // loop bodies: iterations are only recorded per solver, not per method; a simulation
         // normally uses one method, so attribute them to the method that has run
-        int m = s->graph_steps[0] > 0 ? 0 : 1;
-        n += s->graph_steps[0] * s->fixed_nodes[0] + s->graph_steps[1] * s->fixed_nodes[1];
+        int m = s->graph_steps[0] > 0 ? 0 : (s->graph_steps[2] > 0 ? 2 : 1);
+        n += s->graph_steps[0] * s->fixed_nodes[0] + s->graph_steps[1] * s->fixed_nodes[1] + s->graph_steps[2] * s->fixed_nodes[2];
         // the divergence and density loops are peeled: their WHILE bodies run (iterations - 1) times per step
-        const long long steps = s->graph_steps[0] + s->graph_steps[1];
+        const long long steps = s->graph_steps[0] + s->graph_steps[1] + s->graph_steps[2];
         const long long body_v = st.total_it_v > steps ? st.total_it_v - steps : 0;
         const long long body_d = st.total_it_d > steps ? st.total_it_d - steps : 0;
         n += body_v * s->body_nodes[m][LOOP_DIV] + body_d * s->body_nodes[m][LOOP_DENS] +
@@ -1032,7 +1076,7 @@ void sph_destroy(SphSim *s)
     if (!s) return;
     DeviceGuard dg(s->device);
     cudaStreamSynchronize(s->stream);
-    for (int m = 0; m < 2; ++m) if (s->exec[m]) cudaGraphExecDestroy(s->exec[m]);
+    for (int m = 0; m < 3; ++m) if (s->exec[m]) cudaGraphExecDestroy(s->exec[m]);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     if (s->pinned) cudaFreeHost(s->pinned);
     for (auto &t : s->timed) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }

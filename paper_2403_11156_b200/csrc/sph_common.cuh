@@ -50,6 +50,7 @@ struct SimConst {
     int has_dynamic;     // any dynamic rigid body
     int warm;            // warm start of both DFSPH solves (reading R27)
     float warm_w;        // omega
+    float pci_k;         // PCISPH: delta dt^2 (reading R28)
 };
 
 // Loop-control block in device memory (one per simulation).  Written by the host only through
@@ -57,6 +58,7 @@ struct SimConst {
 struct DevControl {
     int forced_v, forced_d, forced_cg;   // -1: tolerances decide
     int min_v, max_v, min_d, max_d, max_cg;
+    int min_p, max_p;                    // PCISPH pressure loop (reading R28)
     int enable_div;
     float eta_v, eta_d, cg_tol;
     // running state of the current step

@@ -22,7 +22,7 @@
 
 namespace sph {
 
-enum { MODE_DIV = 0, MODE_DENS = 1 };
+enum { MODE_DIV = 0, MODE_DENS = 1, MODE_PCI = 2 };   // MODE_PCI: PCISPH pressure loop (reading R28)
 
 struct __align__(32) PV { float4 x, v; };   // position (x, y, z, -) | velocity (vx, vy, vz, rho)
 
@@ -280,7 +280,7 @@ template <int MODE>
 __device__ __forceinline__ void solver_ctrl_eval(double err, DevControl *ctl, DevStats *st, LoopHandle lh, bool first)
 {
     const bool on = MODE == MODE_DIV ? (ctl->enable_div && ctl->forced_v != 0 && ctl->max_v > 0)
-                                     : (ctl->forced_d != 0 && ctl->max_d > 0);
+                  : MODE == MODE_DENS ? (ctl->forced_d != 0 && ctl->max_d > 0) : (ctl->forced_d != 0 && ctl->max_p > 0);
     if (!on) {
         // loop switched off: the peeled first iteration runs with kappa = 0 (a no-op on v)
         if (MODE == MODE_DIV) { st->it_v = 0; st->err_v = 0.f; } else { st->it_d = 0; st->err_rho = 0.f; }
@@ -298,7 +298,8 @@ __device__ __forceinline__ void solver_ctrl_eval(double err, DevControl *ctl, De
         if (f < 0 && !cont && err > (double)ctl->eta_v) st->max_iter_hit |= 1;
     } else {
         int f = ctl->forced_d;
-        cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_d || l < ctl->min_d) && l < ctl->max_d);
+        const int mn = MODE == MODE_PCI ? ctl->min_p : ctl->min_d, mx = MODE == MODE_PCI ? ctl->max_p : ctl->max_d;
+        cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_d || l < mn) && l < mx);
         st->it_d = l; st->err_rho = (float)err;
         if (f < 0 && !cont && err > (double)ctl->eta_d) st->max_iter_hit |= 2;
     }
@@ -450,7 +451,17 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
         float D = c.grad_c * fmaf(c.m, df, db);
         const float dt = step_dt(c);
         float rho = vi.w, a = alpha[i], kappa;
-        if (MODE == MODE_DIV) {
+        if (MODE == MODE_PCI) {
+            // reading R28: rho* = rho + dt D (Eq. 9), p <- max(p + delta (rho* - rho0), 0), delta = pci_k / dt^2;
+            // the C-pass applies the INCREMENT of p / rho^2 (the pressure force of Eq. 7 is linear in p)
+            const float e = fmaf(dt, D, rho) - c.rho0;
+            term = fmaxf(e, 0.f);
+            const float pold = ksum[i];
+            float pn = fmaxf(fmaf(c.pci_k / (dt * dt), e, pold), 0.f);
+            if (first && !(ctl->forced_d != 0 && ctl->max_p > 0)) pn = pold;
+            ksum[i] = pn;
+            kappa = (pn - pold) / rho;                              // written below as kappa / rho = dp / rho^2
+        } else if (MODE == MODE_DIV) {
             term = fmaxf(D, 0.f);
             kappa = a * term / dt;
             // (warm-start path only: there this launch opens the divergence loop, which may be switched off)
@@ -463,7 +474,7 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
             if (first && !(ctl->forced_d != 0 && ctl->max_d > 0)) kappa = 0.f;
         }
         posk[i] = make_float4(xi.x, xi.y, xi.z, kappa / rho);
-        if (ksum != nullptr) ksum[i] += kappa;                     // running total of the solve (warm start, R27)
+        if (MODE != MODE_PCI && ksum != nullptr) ksum[i] += kappa; // running total of the solve (warm start, R27)
     }
     solver_tail<MODE>(c, term, ctl, st, lh, first != 0);
 }
@@ -717,6 +728,24 @@ k_wcsph_eos(SimConst c, const float4 *__restrict__ pos, const float *__restrict_
     float delta = (rt - c.rho0) / c.rho0;
     float pr = c.wc_k * expm1f(c.wc_gamma * log1pf(delta));
     posk[i] = make_float4(x.x, x.y, x.z, pr / (rt * rt));
+}
+
+// PCISPH (reading R28), start of the pressure stage: the record's fourth velocity lane receives rho (the viscosity
+// sums gather rho_j from it, every P-pass reads rho_i from it), the accumulated pressure restarts at 0, and
+// v* = v + dt g (Alg. 1 l.1-2) unless the explicit-viscosity kernel, which adds gravity itself, follows.
+__global__ void __launch_bounds__(256)
+k_pci_begin(SimConst c, const float *__restrict__ rho, PV *__restrict__ pv, float *__restrict__ pacc, int add_gravity)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= c.nf) return;
+    float4 v = pv[i].v;
+    if (add_gravity) {
+        const float dt = step_dt(c);
+        v.x = fmaf(dt, c.gx, v.x); v.y = fmaf(dt, c.gy, v.y); v.z = fmaf(dt, c.gz, v.z);
+    }
+    v.w = rho[i];
+    pv[i].v = v;
+    pacc[i] = 0.f;
 }
 
 // A9 (symplectic Euler) is the tail of the last C-pass: see k_solver_c, TAIL_DENS / TAIL_WCSPH.

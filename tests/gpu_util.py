@@ -110,6 +110,13 @@ def resync_step(g, o, scene, method="dfsph", dv_floor_per_pass=None):
             o.set_forced_dt(st["dt_last"])      # the GPU's fp32 choice of dt (several values are valid, R20 / R26)
         o.step_dfsph(forced_v=fv, forced_d=st["it_d"], forced_cg=fcg)
         o.set_forced_dt(0.0)
+    elif method == "pcisph":
+        g.sph_step_pcisph(1)
+        st = g.sph_read_stats()
+        if scene.params.get("cfl_factor", 0.0) > 0.0:
+            o.set_forced_dt(st["dt_last"])
+        o.step_pcisph(forced=st["it_d"])        # several counts are valid when err ~ eta (R20)
+        o.set_forced_dt(0.0)
     else:
         g.sph_step_wcsph(1)
         st = g.sph_read_stats()

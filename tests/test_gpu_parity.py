@@ -746,3 +746,67 @@ def test_warm_start_parity_and_fewer_iterations(B, oracle):
     # totals are zero without warm start
     assert float(cold.sph_read_state(B.KSUM_DENSITY).abs().max()) == 0.0
     cold.close()
+
+
+# ------------------------------------------------------------------ NEXT-3: PCISPH (reading R28)
+
+def test_pcisph_step_parity_config0_and_viscous_config1(B, oracle):
+    """sph_step_pcisph against the oracle's PCISPH step from the same state, the oracle forced to the GPU's iteration
+    count: config 0 at full size at several checkpoints of a 60-step run (incl. the wall-contact phase, where the
+    pressure loop does real work), config 1 at reduced size with explicit viscosity (Eq. 15 before the loop)."""
+    sc = scenes.config(0)
+    g, o = make_pair(sc, oracle)
+    worked = 0
+    for cp in (0, 1, 30, 45, 59):
+        done = g.sph_read_stats()["steps_done"]
+        if cp > done:
+            g.sph_step_pcisph(int(cp - done))
+        e, st = resync_step(g, o, sc, method="pcisph", dv_floor_per_pass=2.5e-5)
+        check_errors(e, sc)
+        assert st["it_d"] >= 3 and st["err_rho"] <= 1e-3 and st["nan_count"] == 0 and st["it_v"] == 0
+        # accumulated pressure: kappa_over_rho holds the LAST increment dp / rho^2; the oracle's kr likewise
+        worked += int(o.kappa().max() > 0.0)
+    assert worked >= 2                      # the loop built pressure at the later checkpoints
+    g.close(); o.close()
+    sc = scenes.dam_break((24, 24, 24), (48, 24, 24), steps=30, viscosity_mode=1, kinematic_viscosity=0.01)
+    g, o = make_pair(sc, oracle)
+    g.sph_step_pcisph(20)
+    e, st = resync_step(g, o, sc, method="pcisph", dv_floor_per_pass=2.5e-5)
+    check_errors(e, sc)
+    g.close(); o.close()
+
+
+def test_pcisph_loop_semantics_and_modes(B, oracle):
+    """Forced iteration counts apply to the PCISPH loop; graph == host-driven launches == 27-cell walk bit for bit;
+    implicit viscosity is rejected; every step of a 100-step config-0 run converges and the centre of mass agrees with
+    the DFSPH run of the same scene (two PPE solvers, one physics: PAPER.md:158)."""
+    sc = scenes.config(0)
+    g, o = make_pair(sc, oracle)
+    g.sph_set_forced_iterations(-1, 5, -1)
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_step_pcisph(1)
+    assert g.sph_read_stats()["it_d"] == 5
+    o.step_pcisph(forced=5)
+    check_errors(field_errors(g, o, sc), sc)
+    g.close(); o.close()
+    outs = []
+    for over in (dict(), dict(use_cuda_graph=0), dict(use_neighbor_list=0)):
+        s = B.Sim.from_scene(sc, **over)
+        s.sph_step_pcisph(40)
+        outs.append((np_(s.sph_read_state(B.POS)), np_(s.sph_read_state(B.VEL)), s.sph_read_stats()["total_it_d"]))
+        s.close()
+    for p_, v_, it in outs[1:]:
+        assert np.array_equal(p_, outs[0][0]) and np.array_equal(v_, outs[0][1]) and it == outs[0][2]
+    with pytest.raises(B.SphError):
+        s = B.Sim.from_scene(scenes.viscous_column(scale=0.3, steps=8))
+        s.sph_step_pcisph(1)
+    a, b = B.Sim.from_scene(sc), B.Sim.from_scene(sc)
+    for _ in range(100):
+        a.sph_step_pcisph(1)
+        st = a.sph_read_stats()
+        assert st["err_rho"] <= 1e-3 and st["max_iter_hit"] == 0 and st["nan_count"] == 0 and st["overflow_count"] == 0
+    b.sph_step_dfsph(100)
+    ca = np_(a.sph_read_state(B.POS)).astype(np.float64).mean(0)
+    cb = np_(b.sph_read_state(B.POS)).astype(np.float64).mean(0)
+    assert np.linalg.norm(ca - cb) <= 0.25 * 2 * sc.params["particle_radius"]
+    a.close(); b.close()
