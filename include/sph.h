@@ -246,6 +246,29 @@ long long sph_launch_count(SphSim *sim);
 int sph_enable_kernel_timing(SphSim *sim, int enable);
 int sph_read_kernel_times(SphSim *sim, char *buf, size_t bytes);
 
+/* Post-processing stage as CUDA kernels (section 4.3: surface reconstruction of the fluid particles;
+ * the paper uses an external tool and prints no equations -- reading R29): the SPH colour field
+ *   phi(g) = sum_i (m / rho_i) W(|g - x_i|, h)          (cubic spline of reading R1, strict support |g - x_i| < h)
+ * on the nodes g = grid_min + (ix, iy, iz) * cube_size (fp32) of a regular grid of dims[0] x dims[1] x dims[2] nodes,
+ * then marching cubes on its cells: a corner is inside when phi > iso, vertices by linear interpolation from the
+ * edge's lower-index corner, triangles (outward normals) from a case table generated by face tracing.  Particles and
+ * densities are those of the sorted store of the last sph_build_grid / start of the last step (SPH_ESTATE otherwise).
+ *   workspace   DEVICE, >= sph_surface_workspace_bytes() bytes, 256-byte aligned; on return its first
+ *               dims[0]*dims[1]*dims[2] floats hold phi (x fastest, then y, then z);
+ *   triangles   DEVICE, max_triangles * 9 floats: triangle t = vertices (x, y, z) x 3, in cell order (cells x fastest),
+ *               the triangles of a cell in table order; triangles beyond max_triangles are dropped;
+ *   n_triangles HOST (may be NULL): total number of triangles of the surface; when given, the call synchronises.
+ * Asynchronous on the simulation's stream otherwise.  Deterministic (no atomics). */
+typedef struct SphSurfaceParams {
+    float grid_min[3];
+    int   dims[3];        /* nodes per axis, >= 2 each */
+    float cube_size;
+    float iso;            /* surface threshold on phi (the usual choice is ~0.6) */
+} SphSurfaceParams;
+size_t sph_surface_workspace_bytes(const SphSurfaceParams *params);
+int sph_surface_extract(SphSim *sim, const SphSurfaceParams *params, void *workspace, size_t workspace_bytes,
+                        float *triangles, long long max_triangles, long long *n_triangles);
+
 const char *sph_last_error(const SphSim *sim);
 void sph_destroy(SphSim *sim);
 

@@ -26,7 +26,7 @@ SPH_OK, SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA, SPH_EDOMAIN, SPH_ESTATE = 0, -1, -2, 
 EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid", "sph_step_dfsph",
            "sph_step_wcsph", "sph_step_pcisph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
            "sph_read_stats", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
-           "sph_last_error", "sph_destroy"]
+           "sph_surface_workspace_bytes", "sph_surface_extract", "sph_last_error", "sph_destroy"]
 
 
 class SphParams(C.Structure):
@@ -78,6 +78,10 @@ class SphStats(C.Structure):
     ]
 
 
+class SphSurfaceParams(C.Structure):
+    _fields_ = [("grid_min", C.c_float * 3), ("dims", C.c_int * 3), ("cube_size", C.c_float), ("iso", C.c_float)]
+
+
 class SphError(RuntimeError):
     def __init__(self, code: int, text: str):
         super().__init__(f"libsph_b200 error {code}: {text}")
@@ -114,6 +118,10 @@ def load() -> C.CDLL:
         L.sph_launch_count.argtypes = [C.c_void_p]
         L.sph_enable_kernel_timing.argtypes = [C.c_void_p, C.c_int]
         L.sph_read_kernel_times.argtypes = [C.c_void_p, C.c_char_p, C.c_size_t]
+        L.sph_surface_workspace_bytes.restype = C.c_size_t
+        L.sph_surface_workspace_bytes.argtypes = [C.POINTER(SphSurfaceParams)]
+        L.sph_surface_extract.argtypes = [C.c_void_p, C.POINTER(SphSurfaceParams), C.c_void_p, C.c_size_t, C.c_void_p,
+                                          C.c_longlong, C.POINTER(C.c_longlong)]
         L.sph_last_error.restype = C.c_char_p
         L.sph_last_error.argtypes = [C.c_void_p]
         L.sph_destroy.argtypes = [C.c_void_p]
@@ -334,6 +342,35 @@ class Sim:
             name, n, ms = line.split()
             out[name] = (int(n), float(ms))
         return out
+
+    def sph_surface_extract(self, grid_min, dims, cube_size: float, iso: float = 0.6, max_triangles: int = 0):
+        """Colour field + marching cubes (include/sph.h).  Returns (phi [nz, ny, nx] CUDA tensor, triangles
+        [n, 3, 3] CUDA tensor, n_total); with max_triangles = 0 a first call counts the triangles and a second one
+        emits exactly that many."""
+        t = self._torch
+        sp = SphSurfaceParams()
+        sp.grid_min = (C.c_float * 3)(*[float(v) for v in grid_min])
+        sp.dims = (C.c_int * 3)(*[int(v) for v in dims])
+        sp.cube_size = float(cube_size); sp.iso = float(iso)
+        nbytes = int(load().sph_surface_workspace_bytes(C.byref(sp)))
+        if nbytes == 0:
+            raise SphError(SPH_EINVAL, "sph_surface_workspace_bytes rejected the grid")
+        ws = t.empty(nbytes + 256, dtype=t.uint8, device=self.device)
+        off = (-ws.data_ptr()) % 256
+        wptr = ws.data_ptr() + off
+        self._stream.wait_stream(t.cuda.current_stream(self.device))
+        ws.record_stream(self._stream)
+        n = C.c_longlong(0)
+        if max_triangles <= 0:
+            self._check(load().sph_surface_extract(self._h, C.byref(sp), C.c_void_p(wptr), nbytes, None, 0, C.byref(n)))
+            max_triangles = int(n.value)
+        tris = t.empty((max(max_triangles, 1), 3, 3), dtype=t.float32, device=self.device)
+        tris.record_stream(self._stream)
+        self._check(load().sph_surface_extract(self._h, C.byref(sp), C.c_void_p(wptr), nbytes,
+                                               C.c_void_p(tris.data_ptr()), max_triangles, C.byref(n)))
+        nn = int(dims[0]) * int(dims[1]) * int(dims[2])
+        phi = ws[off:off + 4 * nn].view(t.float32).reshape(int(dims[2]), int(dims[1]), int(dims[0]))
+        return self._after_read(phi), self._after_read(tris[:min(int(n.value), max_triangles)]), int(n.value)
 
     def sph_launch_count(self) -> int:
         return int(load().sph_launch_count(self._h))

@@ -14,6 +14,7 @@
 #include "sph_passes.cuh"
 #include "sph_lists.cuh"
 #include "sph_rigid.cuh"
+#include "sph_surface.cuh"
 
 using namespace sph;
 
@@ -1066,6 +1067,75 @@ int sph_read_kernel_times(SphSim *s, char *buf, size_t bytes)
     for (auto &a : acc) { char line[160]; snprintf(line, sizeof line, "%s %lld %.6f\n", a.name.c_str(), a.n, a.ms); out += line; }
     if (out.size() + 1 > bytes) { s->err = "buffer too small"; return SPH_ENOMEM; }
     memcpy(buf, out.c_str(), out.size() + 1);
+    return SPH_OK;
+}
+
+// ---- post-processing stage (sph_surface.cuh)
+namespace {
+struct SurfLayout { size_t field, count, tiles, total; long long nnodes, ncells; int ntiles; };
+bool surf_layout(const SphSurfaceParams *p, SurfLayout &L)
+{
+    if (!p || p->dims[0] < 2 || p->dims[1] < 2 || p->dims[2] < 2 || !(p->cube_size > 0.f)) return false;
+    L.nnodes = (long long)p->dims[0] * p->dims[1] * p->dims[2];
+    L.ncells = (long long)(p->dims[0] - 1) * (p->dims[1] - 1) * (p->dims[2] - 1);
+    if (L.nnodes > 2000000000LL) return false;
+    L.ntiles = cdiv(L.ncells + 1, kScanTile);
+    auto up = [](size_t b) { return (b + 255) & ~size_t(255); };
+    L.field = 0;
+    L.count = up((size_t)L.nnodes * sizeof(float));
+    L.tiles = L.count + up(((size_t)L.ncells + 1 + 4) * sizeof(int));
+    L.total = L.tiles + up((size_t)L.ntiles * sizeof(int));
+    return true;
+}
+bool g_mc_table_ready[64] = { false };
+}  // namespace
+
+size_t sph_surface_workspace_bytes(const SphSurfaceParams *p)
+{
+    SurfLayout L;
+    return surf_layout(p, L) ? L.total : 0;
+}
+
+int sph_surface_extract(SphSim *s, const SphSurfaceParams *sp, void *workspace, size_t workspace_bytes,
+                        float *triangles, long long max_triangles, long long *n_triangles)
+{
+    if (!s) return SPH_EINVAL;
+    SurfLayout L;
+    if (!surf_layout(sp, L)) { s->err = "surface grid needs >= 2 nodes per axis, cube_size > 0 and < 2^31 nodes"; return SPH_EINVAL; }
+    if (!workspace || workspace_bytes < L.total) { s->err = "surface workspace too small"; return SPH_ENOMEM; }
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0) { s->err = "surface workspace must be 256-byte aligned"; return SPH_EINVAL; }
+    if (max_triangles < 0 || (max_triangles > 0 && !triangles)) { s->err = "triangles is NULL"; return SPH_EINVAL; }
+    if (!s->derived_valid) { s->err = "the surface is extracted from the sorted store of the last sph_build_grid / step: call sph_build_grid first"; return SPH_ESTATE; }
+    DeviceGuard dg(s->device);
+    cudaStream_t st = s->stream;
+    if (s->device >= 0 && s->device < 64 && !g_mc_table_ready[s->device]) {
+        unsigned char cnt[256], edg[256 * kMcMaxTris * 3];
+        memset(edg, 0, sizeof edg);
+        if (!mc_build_table(cnt, edg)) { s->err = "marching-cubes table generation failed"; return SPH_ESTATE; }
+        CUDA_TRY(s, cudaMemcpyToSymbol(c_mc_count, cnt, sizeof cnt));
+        CUDA_TRY(s, cudaMemcpyToSymbol(c_mc_edges, edg, sizeof edg));
+        g_mc_table_ready[s->device] = true;
+    }
+    char *base = static_cast<char *>(workspace);
+    float *phi = reinterpret_cast<float *>(base + L.field);
+    int *count = reinterpret_cast<int *>(base + L.count);
+    int *tiles = reinterpret_cast<int *>(base + L.tiles);
+    SurfGrid sg;
+    sg.gx = sp->grid_min[0]; sg.gy = sp->grid_min[1]; sg.gz = sp->grid_min[2]; sg.cs = sp->cube_size; sg.iso = sp->iso;
+    sg.nx = sp->dims[0]; sg.ny = sp->dims[1]; sg.nz = sp->dims[2];
+    LAUNCH(s, k_surface_field, cdiv(L.nnodes, kBlock), kBlock, st, s->c, sg, s->posB, s->rho, s->gf.cell_start, phi);
+    LAUNCH(s, k_surface_classify, cdiv(L.ncells + 1, 256), 256, st, sg, phi, count, L.ncells);
+    const int nscan = (int)(L.ncells + 1);
+    LAUNCH(s, k_scan_tile_sums, L.ntiles, kScanThreads, st, count, nscan, tiles);
+    LAUNCH(s, k_scan_tile_offsets, 1, 1024, st, tiles, L.ntiles);
+    LAUNCH(s, k_scan_apply, L.ntiles, kScanThreads, st, count, nscan, tiles);
+    if (max_triangles > 0)
+        LAUNCH(s, k_surface_emit, cdiv(L.ncells, 256), 256, st, sg, phi, count, L.ncells, triangles, max_triangles);
+    if (n_triangles) {
+        CUDA_TRY(s, cudaMemcpyAsync(s->pinned, count + L.ncells, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(s, cudaStreamSynchronize(st));
+        *n_triangles = s->pinned[0];
+    }
     return SPH_OK;
 }
 

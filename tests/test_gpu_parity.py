@@ -810,3 +810,90 @@ def test_pcisph_loop_semantics_and_modes(B, oracle):
     cb = np_(b.sph_read_state(B.POS)).astype(np.float64).mean(0)
     assert np.linalg.norm(ca - cb) <= 0.25 * 2 * sc.params["particle_radius"]
     a.close(); b.close()
+
+
+# ------------------------------------------------------------------ NEXT-4: post-processing (reading R29)
+
+def _field_brute(pos, vol, h, nodes):
+    """phi at a few nodes by brute force over ALL particles (numpy, fp64; no grid of any kind)."""
+    from oracle import surface_ref as SR
+    out = np.zeros(len(nodes))
+    for k, g in enumerate(nodes):
+        r = np.linalg.norm(pos - g, axis=1)
+        m = r < h
+        out[k] = (vol[m] * SR.kernel_w(r[m], h)).sum()
+    return out
+
+
+def test_surface_field_and_marching_cubes_parity(B, oracle):
+    """sph_surface_extract on a disordered config-0 state: the colour field matches the oracle's (fp64, particle loop) on
+    every node; the triangles equal the oracle's marching cubes run on the SAME fp32 field (inside / outside decisions on
+    identical numbers): same count, same cell order, vertices to fp32 rounding; the mesh is a closed, outward-oriented
+    2-manifold whose volume is the fluid's; two extractions are bit-identical; truncation and state errors behave."""
+    from oracle import surface_ref as SR
+    sc = scenes.config(0)
+    g = B.Sim.from_scene(sc)
+    g.sph_step_dfsph(40)
+    g.sph_build_grid()                      # the surface is taken from the sorted store: make it the current state
+    prm = sc.params
+    h, r = prm["support_radius"], prm["particle_radius"]
+    cs = 1.5 * r
+    gmin = tuple(float(v) - h for v in prm["tank_min"])
+    dims = tuple(int(np.ceil((prm["tank_max"][a] - prm["tank_min"][a] + 2 * h) / cs)) + 1 for a in range(3))
+    phi, tris, n = g.sph_surface_extract(gmin, dims, cs, iso=0.6)
+    assert n == len(tris) and n > 1000
+    pos = np_(g.sph_read_state(B.POS)).astype(np.float64)
+    rho = np_(g.sph_read_state(B.DENSITY)).astype(np.float64)
+    m = prm["rest_density"] * (2 * r) ** 3
+    ref = SR.scalar_field(pos, m / rho, h, gmin, dims, cs)
+    phi_np = np_(phi)
+    assert phi_np.shape == ref.shape
+    assert np.abs(phi_np - ref).max() <= 2e-5 and ref.max() > 0.9
+    ot, oc = SR.marching_cubes(phi_np, 0.6, gmin, cs)
+    tg = np_(tris).astype(np.float64)
+    assert tg.shape == ot.shape
+    assert np.abs(tg - ot).max() <= 5e-7
+    V, E, F, closed = SR.mesh_topology(tg, decimals=6)
+    assert closed
+    vol, area = SR.mesh_volume_area(tg)
+    assert vol == pytest.approx(sc.n_fluid * m / prm["rest_density"], rel=0.08)      # iso 0.6 sits a little outside the outermost particles
+    phi2, tris2, n2 = g.sph_surface_extract(gmin, dims, cs, iso=0.6)
+    assert n2 == n and torch.equal(tris2, tris) and torch.equal(phi2, phi)
+    _, tr3, n3 = g.sph_surface_extract(gmin, dims, cs, iso=0.6, max_triangles=100)
+    assert n3 == n and len(tr3) == 100 and torch.equal(tr3, tris[:100])
+    g.sph_write_state(B.POS, g.sph_read_state(B.POS))
+    with pytest.raises(B.SphError):
+        g.sph_surface_extract(gmin, dims, cs)
+    g.close()
+
+
+def test_surface_full_size_config4(B, oracle):
+    """The stage at the headline size (1.23M particles, the whole 4 x 2 x 2 m tank at cube_size = 2r: 16M nodes): field on
+    a seeded sample of nodes against a brute force over ALL particles, triangle count stable between two runs, enclosed
+    volume = the fluid's."""
+    sc = scenes.config(4)
+    g = B.Sim.from_scene(sc)
+    g.sph_step_dfsph(20)
+    g.sph_build_grid()
+    prm = sc.params
+    h, r = prm["support_radius"], prm["particle_radius"]
+    cs = 2 * r
+    gmin = tuple(float(v) - h for v in prm["tank_min"])
+    dims = tuple(int(np.ceil((prm["tank_max"][a] - prm["tank_min"][a] + 2 * h) / cs)) + 1 for a in range(3))
+    phi, tris, n = g.sph_surface_extract(gmin, dims, cs, iso=0.6)
+    assert n == len(tris) and n > 100000
+    from oracle import surface_ref as SR
+    pos = np_(g.sph_read_state(B.POS)).astype(np.float64)
+    rho = np_(g.sph_read_state(B.DENSITY)).astype(np.float64)
+    m = prm["rest_density"] * (2 * r) ** 3
+    rng = np.random.default_rng(7)
+    inside = torch.nonzero(phi > 0.05)
+    pick = inside[torch.as_tensor(rng.choice(len(inside), 150, replace=False), device=inside.device)]
+    pick = np_(pick)
+    nodes = SR.grid_nodes(gmin, dims, cs)[pick[:, 0], pick[:, 1], pick[:, 2]]
+    ref = _field_brute(pos, m / rho, h, nodes)
+    got = np_(phi)[pick[:, 0], pick[:, 1], pick[:, 2]]
+    assert np.abs(got - ref).max() <= 2e-5
+    vol, _ = SR.mesh_volume_area(np_(tris).astype(np.float64))
+    assert vol == pytest.approx(sc.n_fluid * m / prm["rest_density"], rel=0.05)
+    g.close()
