@@ -897,3 +897,72 @@ def test_surface_full_size_config4(B, oracle):
     vol, _ = SR.mesh_volume_area(np_(tris).astype(np.float64))
     assert vol == pytest.approx(sc.n_fluid * m / prm["rest_density"], rel=0.05)
     g.close()
+
+
+# ------------------------------------------------------------------ degenerate pile-ups (R12 note, list-format limits)
+
+def _clusters(centres, n_each, spread, seed=0):
+    rng = np.random.default_rng(seed)
+    return np.concatenate([np.asarray(c) + rng.uniform(-spread, spread, size=(n_each, 3)) for c in centres])
+
+
+def _scene_from_points(pts, pad):
+    sc = scenes.random_cloud(len(pts), (1.0, 1.0, 1.0), seed=0)
+    sc.fluid_pos = np.ascontiguousarray(pts, dtype=np.float32)
+    sc.fluid_vel = np.zeros_like(sc.fluid_pos)
+    sc.params["domain_min"] = (0.0, 0.0, 0.0)
+    sc.params["domain_max"] = tuple(float(v) for v in pad)
+    sc.params["tank_min"] = sc.params["domain_min"]; sc.params["tank_max"] = sc.params["domain_max"]
+    return sc
+
+
+def test_more_than_2048_particles_in_one_fine_cell(B, oracle):
+    """The only ordering path that is not canonical (k_reorder keeps arrival order in cells above kBigCell = 2048,
+    DESIGN.md R12) and a blown-up state in general: 2600 particles inside ONE fine cell.  Documented behaviour: the
+    grid (cell_start, keys) is still bit-exact, the sorted ids are a permutation, every particle's neighbour list
+    overflows and is counted (the step's results are invalid), the true neighbour maximum is reported, nothing
+    crashes."""
+    h = 0.04
+    c = h * (1 + 2.0 ** -10)
+    pts = _clusters([(2.25 * c, 2.5 * c, 2.5 * c)], 2600, 0.2 * c * np.array([1.0, 2.0, 2.0]), seed=1)
+    pts = np.concatenate([pts, _clusters([(4.6 * c, 2.5 * c, 2.5 * c)], 300, 0.4 * c, seed=2)])
+    sc = _scene_from_points(pts, (7 * c, 5 * c, 5 * c))
+    g, o = make_pair(sc, oracle, max_fluid_neighbors=768)
+    g.sph_build_grid(); o.build_grid()
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_OF_PARTICLE)), o.cell_of_particle(0))
+    cs = o.cell_start(0)
+    assert np.diff(cs).max() >= 2600                      # > kBigCell in one R11 cell, all in one of its two fine slabs
+    assert np.array_equal(np.sort(np_(g.sph_read_state(B.SORTED_ID))), np.arange(g.nf))
+    st = g.sph_read_stats()
+    fs, _ = o.neighbors(0)
+    true_counts = np.diff(fs)
+    assert st["max_fluid_neighbors"] == true_counts.max() and true_counts.max() > 2048
+    assert st["overflow_count"] == int((true_counts > 768).sum()) and st["overflow_count"] >= 2600
+    # particles whose lists did fit still have the exact sets
+    cnt = np_(g.sph_read_state(B.NEIGHBOR_COUNT))[:, 0]
+    assert np.array_equal(np.minimum(true_counts, 768), cnt)
+    g.close(); o.close()
+
+
+def test_run_longer_than_4096_particles_is_flagged(B, oracle):
+    """16-bit list entries hold a 12-bit offset inside the x-run: a run of more than 4096 particles cannot be encoded.
+    Six tight clusters of 700 particles, pairwise more than h apart, inside ONE x-run of 2.5 cells (4200 particles):
+    no particle has more than 699 neighbours (the 768-entry lists would fit), yet the builder must flag the particles
+    whose run is too long instead of writing wrong entries.  The grid itself stays bit-exact."""
+    h = 0.04
+    c = h * (1 + 2.0 ** -10)
+    xs = (2.05 * c, 3.25 * c, 4.45 * c)                     # within +-1.25 cells of the middle one
+    yz = ((2.04 * c, 2.04 * c), (2.96 * c, 2.96 * c))       # same cell row, 1.3 h apart
+    centres = [(x, a, b) for x in xs for (a, b) in yz]
+    pts = _clusters(centres, 700, 0.015 * c, seed=3)
+    sc = _scene_from_points(pts, (7 * c, 5 * c, 5 * c))
+    g, o = make_pair(sc, oracle, max_fluid_neighbors=768)
+    g.sph_build_grid(); o.build_grid()
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    fs, _ = o.neighbors(0)
+    assert np.diff(fs).max() == 699                         # lists alone would not overflow
+    st = g.sph_read_stats()
+    assert st["max_fluid_neighbors"] <= 699
+    assert st["overflow_count"] > 0                         # ... the run length does
+    g.close(); o.close()
