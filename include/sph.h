@@ -208,6 +208,57 @@ int sph_step_wcsph(SphSim *sim, int n_steps);
  * viscosity_mode 2 is not combined with this solver (SPH_ESTATE). */
 int sph_step_pcisph(SphSim *sim, int n_steps);
 
+/* ---- Slab mode: x-slab domain decomposition across GPUs (the paper runs on one GPU,
+ * this is the build's own extension for the 4M-8M sweep).  Every rank (or, for tests, every slab of one
+ * device) owns the particles of an x-range and keeps copies ("ghosts") of the neighbouring slabs' particles within h of
+ * the cuts.  A slab is an ordinary simulation created with n_fluid = its CAPACITY, use_cuda_graph = 0 and static
+ * boundaries; per step the caller
+ *   1. selects migrating particles and ghost layers (sph_select_range), exchanges them with the x-neighbours and hands
+ *      the slab its new set (sph_slab_set_particles: owned first, then ghosts);
+ *   2. runs the passes one by one (sph_slab_phase).  A pass computes garbage FOR ghosts (their neighbourhood is
+ *      incomplete); before the next pass reads that field the owners' values replace it: sph_slab_gather on the owner
+ *      (addressed by the ORIGINAL indices the ghost layer was selected with), transfer, sph_slab_scatter on the ghost
+ *      side.  Fields: KR = kappa/rho (written by every P-pass, read by the C-pass), VEL = velocity + density lane
+ *      (written by every C-pass and the viscosity kernel, read by the P-pass / viscosity);
+ *   3. decides each solver loop ONCE for the whole domain: every P-pass leaves the slab's fixed-point error sum over its
+ *      OWNED particles (sph_slab_read_error_sum: 2^-20 units of dt/rho0 * sum R_i or sum E_i / rho0; integer, so the sum
+ *      over slabs does not depend on the partition), the caller adds them up (all-reduce), applies reading R14 and
+ *      writes the result back (sph_slab_set_loop) before the C-pass, whose tail work depends on it.
+ * paper_2403_11156_b200/slabs.py holds that schedule with two exchange back ends (slabs of one device; torch.distributed).
+ * Not supported in slab mode: dynamic bodies, implicit viscosity, warm start, CUDA-graph launches. */
+typedef enum SphSlabPhase {
+    SPH_SLAB_BEGIN = 0,         /* time step, A1-A3, neighbour lists, original-index -> slot map */
+    SPH_SLAB_DENSITY_DIVP = 1,  /* rho, alpha + first divergence P-pass          -> refresh KR, decide the divergence loop */
+    SPH_SLAB_C_DIV = 2,         /* C-pass of the divergence solve (last: + dt g)  -> refresh VEL */
+    SPH_SLAB_P_DIV = 3,         /* further divergence P-pass                      -> refresh KR, decide */
+    SPH_SLAB_VISCOSITY = 4,     /* explicit viscosity, Eq. 15 (no-op otherwise)   -> refresh VEL */
+    SPH_SLAB_P_DENS_FIRST = 5,  /* first density P-pass                           -> refresh KR, decide the density loop */
+    SPH_SLAB_P_DENS = 6,        /* further density P-pass                         -> refresh KR, decide */
+    SPH_SLAB_C_DENS = 7,        /* C-pass of the density solve (last: integrates) -> refresh VEL unless last */
+    SPH_SLAB_END = 8            /* step statistics */
+} SphSlabPhase;
+typedef enum SphSlabField { SPH_SLAB_FIELD_KR = 0, SPH_SLAB_FIELD_VEL = 1 } SphSlabField;
+
+/* pos4 / vel4: DEVICE, (n_owned + n_ghost) x 4 floats (x, y, z, -), owned particles first; <= the capacity of create. */
+int sph_slab_set_particles(SphSim *sim, const float *pos4, const float *vel4, int n_owned, int n_ghost);
+int sph_slab_phase(SphSim *sim, int phase);
+/* out4[k] = field of the particle whose original index is orig_idx[k] (DEVICE arrays, 4 floats per entry). */
+int sph_slab_gather(SphSim *sim, int field, const int *orig_idx, int n, float *out4);
+/* field of the particles with original indices first_orig .. first_orig + n - 1 = in4[k]. */
+int sph_slab_scatter(SphSim *sim, int field, int first_orig, int n, const float *in4);
+int sph_slab_read_error_sum(SphSim *sim, unsigned long long *total_host);   /* synchronises */
+/* mode 0: divergence loop, 1: density loop; cont = another iteration follows this C-pass; it, err: for SphStats. */
+int sph_slab_set_loop(SphSim *sim, int mode, int cont, int it, float err);
+/* Device pointers INTO the workspace: the persistent store after a step (sorted order; 4 floats per particle) and the
+ * original index of every slot (< n_owned: owned).  Valid until the next sph_slab_set_particles. */
+int sph_slab_store(SphSim *sim, const float **pos4, const float **vel4, const int **orig_idx, int *n, int *n_owned);
+/* Deterministic selection (input order kept) of the entries i < n with x_lo <= pos4[i].x < x_hi and, when key != NULL,
+ * key[i] < key_lt: copies pos4 / vel4, the id gid[key ? key[i] : i] and (optionally) i itself.  All arrays DEVICE except
+ * count_host; scratch: >= n + 8 + (n + 1) / 4096 ints.  Synchronises the stream.  Not tied to a simulation. */
+int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, const int *gid, const int *key, int key_lt,
+                     int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
+                     int max_out, int *scratch, size_t scratch_ints, int *count_host);
+
 /* Override the iteration counts of the next steps: -1 = tolerances decide, >= 0 = exactly that
  * many iterations of the divergence solve / density solve / CG.  Takes effect without re-capture.
  * Synchronises the stream. */

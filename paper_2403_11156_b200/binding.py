@@ -26,7 +26,9 @@ SPH_OK, SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA, SPH_EDOMAIN, SPH_ESTATE = 0, -1, -2, 
 EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid", "sph_step_dfsph",
            "sph_step_wcsph", "sph_step_pcisph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
            "sph_read_stats", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
-           "sph_surface_workspace_bytes", "sph_surface_extract", "sph_last_error", "sph_destroy"]
+           "sph_surface_workspace_bytes", "sph_surface_extract", "sph_slab_set_particles", "sph_slab_phase",
+           "sph_slab_gather", "sph_slab_scatter", "sph_slab_read_error_sum", "sph_slab_set_loop", "sph_slab_store",
+           "sph_select_range", "sph_last_error", "sph_destroy"]
 
 
 class SphParams(C.Structure):
@@ -122,6 +124,17 @@ def load() -> C.CDLL:
         L.sph_surface_workspace_bytes.argtypes = [C.POINTER(SphSurfaceParams)]
         L.sph_surface_extract.argtypes = [C.c_void_p, C.POINTER(SphSurfaceParams), C.c_void_p, C.c_size_t, C.c_void_p,
                                           C.c_longlong, C.POINTER(C.c_longlong)]
+        L.sph_slab_set_particles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int]
+        L.sph_slab_phase.argtypes = [C.c_void_p, C.c_int]
+        L.sph_slab_gather.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]
+        L.sph_slab_scatter.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        L.sph_slab_read_error_sum.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong)]
+        L.sph_slab_set_loop.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_float]
+        L.sph_slab_store.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                     C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.sph_select_range.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                       C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                       C.c_void_p, C.c_size_t, C.POINTER(C.c_int)]
         L.sph_last_error.restype = C.c_char_p
         L.sph_last_error.argtypes = [C.c_void_p]
         L.sph_destroy.argtypes = [C.c_void_p]
@@ -371,6 +384,36 @@ class Sim:
         nn = int(dims[0]) * int(dims[1]) * int(dims[2])
         phi = ws[off:off + 4 * nn].view(t.float32).reshape(int(dims[2]), int(dims[1]), int(dims[0]))
         return self._after_read(phi), self._after_read(tris[:min(int(n.value), max_triangles)]), int(n.value)
+
+    # ---- slab mode (include/sph.h): raw device pointers in, argument marshalling only
+    def sph_slab_set_particles(self, pos4, vel4, n_owned: int, n_ghost: int):
+        self._check(load().sph_slab_set_particles(self._h, C.c_void_p(pos4.data_ptr()), C.c_void_p(vel4.data_ptr()),
+                                                  int(n_owned), int(n_ghost)))
+        self.nf = int(n_owned) + int(n_ghost)
+
+    def sph_slab_phase(self, phase: int):
+        self._check(load().sph_slab_phase(self._h, int(phase)))
+
+    def sph_slab_gather(self, field: int, orig_idx, n: int, out4):
+        self._check(load().sph_slab_gather(self._h, int(field), C.c_void_p(orig_idx.data_ptr()), int(n), C.c_void_p(out4.data_ptr())))
+
+    def sph_slab_scatter(self, field: int, first_orig: int, n: int, in4):
+        self._check(load().sph_slab_scatter(self._h, int(field), int(first_orig), int(n), C.c_void_p(in4.data_ptr())))
+
+    def sph_slab_read_error_sum(self) -> int:
+        v = C.c_ulonglong(0)
+        self._check(load().sph_slab_read_error_sum(self._h, C.byref(v)))
+        return int(v.value)
+
+    def sph_slab_set_loop(self, mode: int, cont: int, it: int, err: float):
+        self._check(load().sph_slab_set_loop(self._h, int(mode), int(cont), int(it), float(err)))
+
+    def sph_slab_store(self):
+        """(pos4 ptr, vel4 ptr, orig_idx ptr, n, n_owned): device pointers into the workspace."""
+        a, b, c = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        n, no = C.c_int(0), C.c_int(0)
+        self._check(load().sph_slab_store(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(n), C.byref(no)))
+        return a.value, b.value, c.value, int(n.value), int(no.value)
 
     def sph_launch_count(self) -> int:
         return int(load().sph_launch_count(self._h))

@@ -61,6 +61,9 @@ struct SphSim {
     float *alpha = nullptr, *rho = nullptr;
     float *ksum_v = nullptr, *ksum_d = nullptr;   // warm start: running totals of the step's solves (sorted order)
     float *pacc = nullptr;          // PCISPH: accumulated pressure of the running step (sorted order)
+    int cap = 0;                    // fluid capacity the workspace was laid out for (= n_fluid of sph_create)
+    int *inv = nullptr;             // slab mode: original index -> sorted slot of the running step
+    PV *slab_vcur = nullptr;        // slab mode: the records the density solve works on (pvB, or pvC after explicit viscosity)
     GridBufs gf, gb;
     uint16_t *nl_f = nullptr;       // 16-bit (run, offset) entries, warp-tiled (sph_passes.cuh)
     int *nl_b = nullptr, *ncount = nullptr;
@@ -197,7 +200,7 @@ bool make_const(const SphParams &p, int nf, int nb, SimConst &c, std::string &wh
     }
     if (p.viscosity_mode < 0 || p.viscosity_mode > 2) { why = "viscosity_mode must be 0 (none), 1 (explicit, Eq. 15) or 2 (implicit, Eq. 16-19)"; return false; }
     if (!make_geom(p, c.g, why)) return false;
-    c.nf = nf; c.nb = nb;
+    c.nf = nf; c.nb = nb; c.nown = nf;
     c.kf = list_cap(p.max_fluid_neighbors, kMaxListCap);
     c.kb = list_cap(p.max_boundary_neighbors, 65532);
     c.h = p.support_radius;
@@ -263,6 +266,7 @@ size_t layout(SphSim &s, void *base)
     s.rho = w.take<float>(nf1);
     if (s.prm.warm_start) { s.ksum_v = w.take<float>(nf1); s.ksum_d = w.take<float>(nf1); }
     s.pacc = w.take<float>(nf1);
+    s.inv = w.take<int>(nf1);
     s.gf.n = (int)nf;
     s.gf.key = w.take<int>(nf1); s.gf.off = w.take<int>(nf1); s.gf.slot = w.take<int>(nf1);
     s.gf.cell_start = w.take<int>(s.cs_len);
@@ -322,7 +326,7 @@ PassCtx make_ctx(const SphSim *s)
     p.c = s->c;
     p.pos = s->posB; p.bpos = s->bpos_s;
     p.fcs = s->gf.cell_start; p.bcs = s->gb.cell_start;
-    p.nl_f = s->nl_f; p.nl_b = s->nl_b; p.ncount = s->ncount;
+    p.nl_f = s->nl_f; p.nl_b = s->nl_b; p.ncount = s->ncount; p.id = s->idB;
     return p;
 }
 
@@ -800,6 +804,7 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
     s->prm = *params;
     s->nbodies = n_bodies;
     s->device = cuda_device;
+    s->cap = n_fluid;
     s->stream = static_cast<cudaStream_t>(cuda_stream);
     s->cur_counter = &s->misc_launches;
     auto fail = [&](int code) { g_create_error = s->err; if (s->cap_stream) cudaStreamDestroy(s->cap_stream); if (s->pinned) cudaFreeHost(s->pinned); delete s; return code; };
@@ -937,6 +942,175 @@ int sph_build_grid(SphSim *s)
 int sph_step_dfsph(SphSim *s, int n_steps) { return do_steps(s, 0, n_steps); }
 int sph_step_wcsph(SphSim *s, int n_steps) { return do_steps(s, 1, n_steps); }
 int sph_step_pcisph(SphSim *s, int n_steps) { return do_steps(s, 2, n_steps); }
+
+// ---- slab mode: the pieces of a DFSPH step as separate calls, so that the caller can
+// refresh the ghost particles between the passes and decide the loops from the error sums of ALL slabs
+}  // extern "C"
+namespace {
+int slab_check(SphSim *s)
+{
+    if (!s) return SPH_EINVAL;
+    if (s->prm.use_cuda_graph) { s->err = "slab mode drives the passes from the host: create the simulation with use_cuda_graph = 0"; return SPH_ESTATE; }
+    if (s->c.has_dynamic) { s->err = "slab mode supports static boundaries only"; return SPH_ESTATE; }
+    if (s->prm.viscosity_mode == 2 || s->prm.warm_start) { s->err = "slab mode: implicit viscosity and warm start are not supported"; return SPH_ESTATE; }
+    if (s->prm.cfl_factor > 0.f) { s->err = "slab mode: the CFL-adaptive time step needs a global velocity maximum and is not supported"; return SPH_ESTATE; }
+    return SPH_OK;
+}
+template <bool LIST>
+int slab_phase_t(SphSim *s, int phase)
+{
+    cudaStream_t st = s->stream;
+    LoopCtx plain{ st, 0, 0 };
+    const int nf = s->c.nf;
+    switch (phase) {
+    case SPH_SLAB_BEGIN: {
+        LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl, s->prm.cfl_factor * 2.0f * s->prm.particle_radius, s->prm.dt_min, s->prm.dt);
+        int rc = enqueue_fluid_grid_and_lists(s, st);
+        if (rc) return rc;
+        if (nf > 0) LAUNCH(s, k_slab_inverse, cdiv(nf, 256), 256, st, s->idB, nf, s->inv);
+        s->slab_vcur = s->pvB;
+        return SPH_OK;
+    }
+    case SPH_SLAB_DENSITY_DIVP: return enqueue_density(s, plain, true);
+    case SPH_SLAB_C_DIV: return nf > 0 ? enqueue_solver_c<LIST>(s, st, TAIL_DIV, s->pvB) : (int)SPH_OK;
+    case SPH_SLAB_P_DIV: return nf > 0 ? enqueue_solver_p<LIST>(s, plain, MODE_DIV, s->pvB, 0) : (int)SPH_OK;
+    case SPH_SLAB_VISCOSITY:
+        if (s->prm.viscosity_mode == 1 && nf > 0) {
+            PassCtx p = make_ctx(s);
+            LAUNCH(s, (k_explicit_viscosity<LIST, false>), s->nblocks, kBlock, st, p, s->pvB, s->pvC);
+            s->slab_vcur = s->pvC;
+        }
+        return SPH_OK;
+    case SPH_SLAB_P_DENS_FIRST: return nf > 0 ? enqueue_solver_p<LIST>(s, plain, MODE_DENS, s->slab_vcur, 1) : (int)SPH_OK;
+    case SPH_SLAB_P_DENS: return nf > 0 ? enqueue_solver_p<LIST>(s, plain, MODE_DENS, s->slab_vcur, 0) : (int)SPH_OK;
+    case SPH_SLAB_C_DENS: return nf > 0 ? enqueue_solver_c<LIST>(s, st, TAIL_DENS, s->slab_vcur) : (int)SPH_OK;
+    case SPH_SLAB_END:
+        LAUNCH(s, k_step_end, 1, 1, st, s->stats, s->ctl);
+        s->derived_valid = true; s->vmax_valid = true;
+        return SPH_OK;
+    default: s->err = "unknown slab phase"; return SPH_EINVAL;
+    }
+}
+}  // namespace
+extern "C" {
+
+int sph_slab_set_particles(SphSim *s, const float *pos4, const float *vel4, int n_owned, int n_ghost)
+{
+    int rc = slab_check(s);
+    if (rc) return rc;
+    const long long n = (long long)n_owned + n_ghost;
+    if (n_owned < 0 || n_ghost < 0 || n > s->cap) { char b[160]; snprintf(b, sizeof b, "slab particle count %lld exceeds the capacity %d the simulation was created with", n, s->cap); s->err = b; return SPH_ENOMEM; }
+    if (n > 0 && (!pos4 || !vel4)) { s->err = "pos4 / vel4 is NULL"; return SPH_EINVAL; }
+    DeviceGuard dg(s->device);
+    cudaStream_t st = s->stream;
+    s->c.nf = (int)n; s->c.nown = n_owned;
+    s->gf.n = (int)n;
+    s->nblocks = cdiv(n > 0 ? n : 1, kBlock);
+    if (n > 0) {
+        CUDA_TRY(s, cudaMemcpyAsync(s->posA, pos4, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+        CUDA_TRY(s, cudaMemcpyAsync(s->velA, vel4, sizeof(float4) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+        LAUNCH(s, k_iota, cdiv(n, 256), 256, st, s->idA, (int)n);
+    }
+    // the list builder reads the SoA positions up to 3 elements past the last particle
+    CUDA_TRY(s, cudaMemsetAsync(s->px + n, 0, 4 * sizeof(float), st));
+    CUDA_TRY(s, cudaMemsetAsync(s->py + n, 0, 4 * sizeof(float), st));
+    CUDA_TRY(s, cudaMemsetAsync(s->pz + n, 0, 4 * sizeof(float), st));
+    s->derived_valid = false; s->vmax_valid = false;
+    return SPH_OK;
+}
+
+int sph_slab_phase(SphSim *s, int phase)
+{
+    int rc = slab_check(s);
+    if (rc) return rc;
+    DeviceGuard dg(s->device);
+    return s->prm.use_neighbor_list ? slab_phase_t<true>(s, phase) : slab_phase_t<false>(s, phase);
+}
+
+int sph_slab_gather(SphSim *s, int what, const int *orig_idx, int n, float *out4)
+{
+    int rc = slab_check(s);
+    if (rc) return rc;
+    if (n < 0 || (n > 0 && (!orig_idx || !out4)) || (what != SPH_SLAB_FIELD_KR && what != SPH_SLAB_FIELD_VEL)) { s->err = "sph_slab_gather: bad argument"; return SPH_EINVAL; }
+    if (n == 0) return SPH_OK;
+    DeviceGuard dg(s->device);
+    const float4 *f = what == SPH_SLAB_FIELD_KR ? s->posk : &s->slab_vcur->v;
+    LAUNCH(s, k_slab_gather, cdiv(n, 256), 256, s->stream, f, what == SPH_SLAB_FIELD_KR ? 1 : 2, s->inv, orig_idx, n, reinterpret_cast<float4 *>(out4));
+    return SPH_OK;
+}
+
+int sph_slab_scatter(SphSim *s, int what, int first_orig, int n, const float *in4)
+{
+    int rc = slab_check(s);
+    if (rc) return rc;
+    if (n < 0 || first_orig < 0 || (long long)first_orig + n > s->c.nf || (n > 0 && !in4) || (what != SPH_SLAB_FIELD_KR && what != SPH_SLAB_FIELD_VEL)) { s->err = "sph_slab_scatter: bad argument"; return SPH_EINVAL; }
+    if (n == 0) return SPH_OK;
+    DeviceGuard dg(s->device);
+    float4 *f = what == SPH_SLAB_FIELD_KR ? s->posk : &s->slab_vcur->v;
+    LAUNCH(s, k_slab_scatter, cdiv(n, 256), 256, s->stream, f, what == SPH_SLAB_FIELD_KR ? 1 : 2, s->inv, first_orig, n, reinterpret_cast<const float4 *>(in4));
+    return SPH_OK;
+}
+
+int sph_slab_read_error_sum(SphSim *s, unsigned long long *total)
+{
+    int rc = slab_check(s);
+    if (rc) return rc;
+    if (!total) return SPH_EINVAL;
+    DeviceGuard dg(s->device);
+    unsigned long long *h = reinterpret_cast<unsigned long long *>(s->pinned + 8);
+    *h = 0ull;
+    if (s->c.nf > 0) {
+        CUDA_TRY(s, cudaMemcpyAsync(h, &s->ctl->last_total, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    }
+    *total = *h;
+    return SPH_OK;
+}
+
+int sph_slab_set_loop(SphSim *s, int mode, int cont, int it, float err)
+{
+    int rc = slab_check(s);
+    if (rc) return rc;
+    DeviceGuard dg(s->device);
+    LAUNCH(s, k_slab_set_loop, 1, 1, s->stream, s->ctl, s->stats, mode, cont, it, err);
+    return SPH_OK;
+}
+
+int sph_slab_store(SphSim *s, const float **pos4, const float **vel4, const int **orig_idx, int *n, int *n_owned)
+{
+    if (!s) return SPH_EINVAL;
+    if (pos4) *pos4 = reinterpret_cast<const float *>(s->posA);
+    if (vel4) *vel4 = reinterpret_cast<const float *>(s->velA);
+    if (orig_idx) *orig_idx = s->idA;
+    if (n) *n = s->c.nf;
+    if (n_owned) *n_owned = s->c.nown;
+    return SPH_OK;
+}
+
+int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, const int *gid, const int *key, int key_lt,
+                     int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
+                     int max_out, int *scratch, size_t scratch_ints, int *count_host)
+{
+    if (n < 0 || max_out < 0 || !scratch || !count_host) return SPH_EINVAL;
+    *count_host = 0;
+    if (n == 0) return SPH_OK;
+    if (!pos4 || !vel4 || !gid || (max_out > 0 && (!out_pos4 || !out_vel4 || !out_gid))) return SPH_EINVAL;
+    const int ntiles = cdiv((long long)n + 1, kScanTile);
+    const size_t flag_len = ((size_t)n + 1 + 3) & ~size_t(3);
+    if (scratch_ints < flag_len + (size_t)ntiles + 4) return SPH_ENOMEM;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int *flag = scratch, *tiles = scratch + flag_len;
+    k_select_flag<<<cdiv((long long)n + 1, 256), 256, 0, st>>>(reinterpret_cast<const float4 *>(pos4), key, key_lt, n, x_lo, x_hi, flag);
+    k_scan_tile_sums<<<ntiles, kScanThreads, 0, st>>>(flag, n + 1, tiles);
+    k_scan_tile_offsets<<<1, 1024, 0, st>>>(tiles, ntiles);
+    k_scan_apply<<<ntiles, kScanThreads, 0, st>>>(flag, n + 1, tiles);
+    if (max_out > 0)
+        k_select_copy<<<cdiv(n, 256), 256, 0, st>>>(reinterpret_cast<const float4 *>(pos4), reinterpret_cast<const float4 *>(vel4), gid, key,
+                                                  flag, n, reinterpret_cast<float4 *>(out_pos4), reinterpret_cast<float4 *>(out_vel4), out_gid, out_idx, max_out);
+    if (cudaMemcpyAsync(count_host, flag + n, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return SPH_ECUDA;
+    if (cudaStreamSynchronize(st) != cudaSuccess) return SPH_ECUDA;
+    return cudaGetLastError() == cudaSuccess ? SPH_OK : SPH_ECUDA;
+}
 
 int sph_set_forced_iterations(SphSim *s, int forced_v, int forced_d, int forced_cg)
 {

@@ -34,6 +34,8 @@ struct Geom {
 struct SimConst {
     Geom g;
     int nf, nb;          // fluid / boundary particle counts
+    int nown;            // slab mode: particles whose original index is < nown are OWNED, the rest are ghosts
+                         // of a neighbouring slab and stay out of the error sums; = nf otherwise
     int kf, kb;          // neighbour-list capacities (rows per warp tile)
     float h, h2, inv_h;  // support radius, h*h in fp32 (R10), 1/h
     float sigma;         // 8 / (pi h^3)           (R1)
@@ -68,6 +70,7 @@ struct DevControl {
     int cg_break;
     float dt;                            // time step of the running step (R26; = SphParams.dt when cfl_factor = 0)
     unsigned long long acc;              // running P-pass: CTA counter (top 20 bits) | fixed-point error sum (A12)
+    unsigned long long last_total;       // fixed-point error sum of the last P-pass (slab mode: summed over the slabs by the host)
 };
 
 // Statistics block in device memory; sph_read_stats copies it out and converts to SphStats.

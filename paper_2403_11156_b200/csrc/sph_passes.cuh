@@ -58,6 +58,7 @@ struct PassCtx {
     uint16_t *nl_f;     // fluid neighbour list, 16-bit (x-run, offset) entries (see below)
     int *nl_b;          // boundary neighbour list, sorted boundary indices
     int *ncount;        // [nf] (#fluid) | (#boundary << 16)
+    const int *id;      // [nf] original index of the particle in sorted slot s (slab mode: owned / ghost)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -316,6 +317,9 @@ __device__ __forceinline__ void solver_ctrl_eval(double err, DevControl *ctl, De
 // 44-bit field cannot carry into the counter (a mean error above ~13 at 1.2M particles saturates).
 constexpr int kAccFracBits = 20, kAccSumBits = 44;
 
+// slab mode: ghosts (copies of a neighbouring slab's particles) do not count in the error sums
+__device__ __forceinline__ bool is_ghost(const PassCtx &p, int i) { return p.c.nown < p.c.nf && p.id[i] >= p.c.nown; }
+
 template <int MODE>
 __device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevControl *ctl, DevStats *st,
                                             LoopHandle lh, bool first)
@@ -331,6 +335,7 @@ __device__ __forceinline__ void solver_tail(const SimConst &c, float term, DevCo
     if ((old >> kAccSumBits) != (unsigned long long)(gridDim.x - 1)) return;
     ctl->acc = 0ull;                                            // every CTA has arrived: reset for the next pass
     unsigned long long total = (old & ((1ull << kAccSumBits) - 1ull)) + q;
+    ctl->last_total = total;
     double err = c.nf > 0 ? (double)total / (double)(1u << kAccFracBits) / (double)c.nf : 0.0;
     solver_ctrl_eval<MODE>(err, ctl, st, lh, first);
 }
@@ -406,6 +411,7 @@ k_density_alpha(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__
             term = fmaxf(D, 0.f);
             float kappa = a * term / step_dt(c);
             posk[i] = make_float4(xi.x, xi.y, xi.z, on ? kappa / rho : 0.f);
+            if (is_ghost(p, i)) term = 0.f;
         }
     }
     if (DIVP) solver_tail<MODE_DIV>(c, term, ctl, st, lh, true);
@@ -475,6 +481,7 @@ k_solver_p(PassCtx p, const PV *__restrict__ pv, const float4 *__restrict__ bvel
         }
         posk[i] = make_float4(xi.x, xi.y, xi.z, kappa / rho);
         if (MODE != MODE_PCI && ksum != nullptr) ksum[i] += kappa; // running total of the solve (warm start, R27)
+        if (is_ghost(p, i)) term = 0.f;
     }
     solver_tail<MODE>(c, term, ctl, st, lh, first != 0);
 }

@@ -111,6 +111,66 @@ k_export_neighbors(const int *__restrict__ nl, const int *__restrict__ ncount, i
 }
 
 // ---------------------------------------------------------------------------------------------
+// Slab mode: x-slab domain decomposition.  A slab's simulation holds its OWNED particles
+// (original indices [0, nown)) followed by GHOSTS, copies of the neighbouring slabs' particles within h of the cut.
+// Ghosts take part in every pass as neighbours; what a pass computes FOR them is wrong (their own neighbourhood is
+// incomplete) and is overwritten with the owner's value before the next pass reads it (gather on the owner's side,
+// scatter on the ghost's side, both addressed by original index through inv[]).
+__global__ void __launch_bounds__(256) k_slab_inverse(const int *__restrict__ id, int n, int *__restrict__ inv)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) inv[id[s]] = s;
+}
+// out[k] = field[inv[idx[k]] * stride]   (float4 elements)
+__global__ void __launch_bounds__(256)
+k_slab_gather(const float4 *__restrict__ field, int stride, const int *__restrict__ inv, const int *__restrict__ idx, int n,
+              float4 *__restrict__ out)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = field[(size_t)inv[idx[k]] * stride];
+}
+// field[inv[first + k] * stride] = in[k]
+__global__ void __launch_bounds__(256)
+k_slab_scatter(float4 *__restrict__ field, int stride, const int *__restrict__ inv, int first, int n, const float4 *__restrict__ in)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) field[(size_t)inv[first + k] * stride] = in[k];
+}
+// loop state decided by the host from the error sums of ALL slabs (reading R14 evaluated once for the whole domain)
+__global__ void k_slab_set_loop(DevControl *ctl, DevStats *st, int mode, int cont, int it, float err)
+{
+    ctl->cont = cont; ctl->it = it;
+    if (mode == 0) { st->it_v = it; st->err_v = err; } else { st->it_d = it; st->err_rho = err; }
+}
+// selection of the particles with lo <= x < hi (and key[i] < key_lt when key != NULL) for migration / ghost layers:
+// flag, exclusive scan (the grid builder's), compacting copy -- deterministic, input order kept
+__global__ void __launch_bounds__(256)
+k_select_flag(const float4 *__restrict__ pos, const int *__restrict__ key, int key_lt, int n, float lo, float hi, int *__restrict__ flag)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    int f = 0;
+    if (i < n) {
+        const float x = pos[i].x;
+        f = (x >= lo && x < hi && (key == nullptr || key[i] < key_lt)) ? 1 : 0;
+    }
+    flag[i] = f;
+}
+__global__ void __launch_bounds__(256)
+k_select_copy(const float4 *__restrict__ pos, const float4 *__restrict__ vel, const int *__restrict__ gid, const int *__restrict__ key,
+              const int *__restrict__ offset, int n, float4 *__restrict__ opos, float4 *__restrict__ ovel, int *__restrict__ ogid,
+              int *__restrict__ oidx, int max_out)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int o = offset[i];
+    if (offset[i + 1] == o || o >= max_out) return;
+    opos[o] = pos[i]; ovel[o] = vel[i];
+    ogid[o] = gid[key != nullptr ? key[i] : i];        // gid is indexed by ORIGINAL index when a key (= original index of slot i) is given
+    if (oidx != nullptr) oidx[o] = i;
+}
+
+// ---------------------------------------------------------------------------------------------
 // Body-frame coordinates and initial sample velocities: xbar_k = R(q)^T (x_k - X),
 // v_k = V + omega x (x_k - X) for dynamic bodies, 0 for static ones.
 __device__ __forceinline__ void quat_to_R(const float q[4], double R[9])

@@ -966,3 +966,82 @@ def test_run_longer_than_4096_particles_is_flagged(B, oracle):
     assert st["max_fluid_neighbors"] <= 699
     assert st["overflow_count"] > 0                         # ... the run length does
     g.close(); o.close()
+
+
+# ------------------------------------------------------------------ NEXT-2: x-slab sharding (one-device emulation)
+
+def _slab_fields(runner, field, B):
+    """{global id: row} of a per-particle field over the OWNED particles of all slabs (rows in local original order)."""
+    out = {}
+    for s in runner.slabs:
+        a = np_(s.sim.sph_read_state(field))
+        gid = np_(s.gid[s.cur])[: s.n_total]
+        for k in range(s.n_owned):
+            out[int(gid[k])] = (a[k], gid)
+    return out
+
+
+@pytest.mark.parametrize("n_slabs", [2, 3])
+def test_slabs_equal_one_domain(B, oracle, n_slabs):
+    """SURVEY 8(e) / NEXT-2 on ONE device: the config-4 scene at 250k particles cut into x-slabs (ghost layers of width
+    h refreshed between the passes, loops decided from the summed error of all slabs, migration every step) against the
+    ordinary single-domain simulation.  First step: every owned particle's neighbour set is bit-exact (as global
+    ids), rho and alpha agree to 1e-5.  After 25 steps (particles have crossed the cuts): same iteration counts, v and
+    x within the 1e-4 bar.  Multi-GPU proper (NCCL back end of the same schedule) is unmeasured on hardware."""
+    from paper_2403_11156_b200 import slabs as S
+    sc = scenes.splash(n_target=250e3)
+    one = B.Sim.from_scene(sc)
+    # (the scene's two blocks are a gap apart: equal halves would never touch; cut inside a block instead)
+    runner, cuts = S.make_local_slabs(sc, n_slabs, fractions=(0.3,) if n_slabs == 2 else None)
+    runner.step()
+    one.sph_step_dfsph(1)
+    st = one.sph_read_stats()
+    assert (runner.stats["it_v"], runner.stats["it_d"]) == (st["it_v"], st["it_d"])
+    assert abs(runner.stats["err_rho"] - st["err_rho"]) <= 1e-6
+    # neighbour sets of the step's start state, as global ids
+    ref_rows = np_(one.sph_read_state(B.FLUID_NEIGHBORS))
+    ref_rho, ref_al = np_(one.sph_read_state(B.DENSITY)), np_(one.sph_read_state(B.ALPHA))
+    checked = 0
+    rng = np.random.default_rng(0)
+    for s in runner.slabs:
+        rows = np_(s.sim.sph_read_state(B.FLUID_NEIGHBORS))
+        rho, al = np_(s.sim.sph_read_state(B.DENSITY)), np_(s.sim.sph_read_state(B.ALPHA))
+        gid = np_(s.gid[s.cur])[: s.n_total].astype(np.int64)
+        assert s.n_total > s.n_owned                                    # it does hold ghosts
+        own_g = gid[: s.n_owned]
+        assert np.abs(rho[: s.n_owned] - ref_rho[own_g]).max() <= 1e-5 * 1000.0
+        assert np.abs(al[: s.n_owned] - ref_al[own_g]).max() <= 1e-5 * np.abs(ref_al).max()
+        # all particles within 2h of a cut plus a random sample of the rest
+        x = sc.fluid_pos[own_g, 0]
+        near = np.zeros(s.n_owned, dtype=bool)
+        for c in cuts[1:-1]:
+            near |= np.abs(x - c) < 2 * sc.params["support_radius"]
+        pick = np.unique(np.concatenate([np.nonzero(near)[0], rng.choice(s.n_owned, 2000, replace=False)]))
+        for k in pick:
+            r = rows[k]
+            mine = frozenset(int(gid[j]) for j in r[r >= 0])
+            rr = ref_rows[own_g[k]]
+            assert mine == frozenset(int(j) for j in rr[rr >= 0])
+        checked += len(pick)
+    assert checked > 6000
+    runner.run(24)                                   # 25 steps x 0.4 mm: particles cross the cuts (lattice planes 10 mm apart)
+    one.sph_step_dfsph(24)
+    st = one.sph_read_stats()
+    assert (runner.stats["total_it_v"], runner.stats["total_it_d"]) == (st["total_it_v"], st["total_it_d"])
+    pos, vel = np_(one.sph_read_state(B.POS)).astype(np.float64), np_(one.sph_read_state(B.VEL)).astype(np.float64)
+    seen = np.zeros(sc.n_fluid, dtype=int)
+    moved = 0
+    vscale = np.linalg.norm(vel, axis=1).max()
+    for k, s in enumerate(runner.slabs):
+        g, p_, v_ = s.owned_state()
+        seen[g] += 1
+        assert np.linalg.norm(v_ - vel[g], axis=1).max() <= 1e-4 * vscale
+        assert np.abs(p_ - pos[g]).max() <= 25 * sc.params["dt"] * 1e-4 * vscale + 1e-6
+        assert (p_[:, 0] >= cuts[k] - 1e-3).all() and (p_[:, 0] < cuts[k + 1] + 1e-3).all()
+        x0 = sc.fluid_pos[g, 0]
+        moved += int(((x0 < cuts[k]) | (x0 >= cuts[k + 1])).sum())
+    assert (seen == 1).all()                                            # every particle owned by exactly one slab
+    assert moved > 0                                                    # ... and some have changed owner
+    for s in runner.slabs:
+        s.close()
+    one.close()
