@@ -308,7 +308,6 @@ int enqueue_grid(SphSim *s, cudaStream_t st, GridBufs &g, const float4 *a_in, co
         LAUNCH(s, k_cell_key_hist, cdiv(g.n, 256), 256, st, a_in, g.n, s->c.g, g.key, g.off, g.cell_start, oob);
     const int nscan = s->c.g.ncells + 1;
     LAUNCH(s, k_scan_tile_sums, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
-    LAUNCH(s, k_scan_tile_offsets, 1, 1024, st, g.tile_sum, g.ntiles);
     LAUNCH(s, k_scan_apply, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
     if (g.n > 0) {
         LAUNCH(s, k_scatter_slots, cdiv(g.n, 256), 256, st, g.key, g.off, g.cell_start, g.n, g.slot);
@@ -1102,7 +1101,6 @@ int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, co
     int *flag = scratch, *tiles = scratch + flag_len;
     k_select_flag<<<cdiv((long long)n + 1, 256), 256, 0, st>>>(reinterpret_cast<const float4 *>(pos4), key, key_lt, n, x_lo, x_hi, flag);
     k_scan_tile_sums<<<ntiles, kScanThreads, 0, st>>>(flag, n + 1, tiles);
-    k_scan_tile_offsets<<<1, 1024, 0, st>>>(tiles, ntiles);
     k_scan_apply<<<ntiles, kScanThreads, 0, st>>>(flag, n + 1, tiles);
     if (max_out > 0)
         k_select_copy<<<cdiv(n, 256), 256, 0, st>>>(reinterpret_cast<const float4 *>(pos4), reinterpret_cast<const float4 *>(vel4), gid, key,
@@ -1301,7 +1299,6 @@ int sph_surface_extract(SphSim *s, const SphSurfaceParams *sp, void *workspace, 
     LAUNCH(s, k_surface_classify, cdiv(L.ncells + 1, 256), 256, st, sg, phi, count, L.ncells);
     const int nscan = (int)(L.ncells + 1);
     LAUNCH(s, k_scan_tile_sums, L.ntiles, kScanThreads, st, count, nscan, tiles);
-    LAUNCH(s, k_scan_tile_offsets, 1, 1024, st, tiles, L.ntiles);
     LAUNCH(s, k_scan_apply, L.ntiles, kScanThreads, st, count, nscan, tiles);
     if (max_triangles > 0)
         LAUNCH(s, k_surface_emit, cdiv(L.ncells, 256), 256, st, sg, phi, count, L.ncells, triangles, max_triangles);
