@@ -102,3 +102,29 @@ def test_product_never_imports_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "sphref" not in txt and "import oracle" not in txt and "from oracle" not in txt, f
+
+
+def test_round2_host_logic_without_a_gpu(binding):
+    """Host-side argument checks and sizing of the round-2 entry points (no compute call is made):
+    warm-start factor range, surface-grid sizing, NULL / size rejection of the selection and slab calls."""
+    sc = scenes.config(0)
+    assert binding.sph_workspace_bytes(binding.make_params(dict(sc.params, warm_start=1, warm_start_factor=1.5)), 10, 0, 0) == 0
+    cold = binding.sph_workspace_bytes(binding.make_params(sc.params), 1000, 0, 0)
+    warm = binding.sph_workspace_bytes(binding.make_params(dict(sc.params, warm_start=1)), 1000, 0, 0)
+    assert warm >= cold + 2 * 4 * 1000                     # the two running-total arrays
+    L = binding.load()
+    sp = binding.SphSurfaceParams()
+    sp.grid_min = (ctypes.c_float * 3)(0, 0, 0); sp.cube_size = 0.01; sp.iso = 0.6
+    sp.dims = (ctypes.c_int * 3)(10, 20, 30)
+    need = L.sph_surface_workspace_bytes(ctypes.byref(sp))
+    assert 4 * 6000 + 4 * 9 * 19 * 29 <= need <= 4 * 6000 + 4 * 9 * 19 * 29 + 4096
+    sp.dims = (ctypes.c_int * 3)(1, 20, 30)                 # fewer than 2 nodes on an axis: no cells
+    assert L.sph_surface_workspace_bytes(ctypes.byref(sp)) == 0
+    sp.dims = (ctypes.c_int * 3)(10, 20, 30); sp.cube_size = 0.0
+    assert L.sph_surface_workspace_bytes(ctypes.byref(sp)) == 0
+    cnt = ctypes.c_int(7)
+    assert L.sph_select_range(None, None, None, None, None, 0, 5, 0.0, 1.0, None, None, None, None, 0, None, 0,
+                              ctypes.byref(cnt)) == binding.SPH_EINVAL      # no scratch
+    assert L.sph_slab_phase(None, 0) == binding.SPH_EINVAL
+    assert L.sph_surface_extract(None, ctypes.byref(sp), None, 0, None, 0, None) == binding.SPH_EINVAL
+    assert L.sph_step_pcisph(None, 1) == binding.SPH_EINVAL

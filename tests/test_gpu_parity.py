@@ -1045,3 +1045,70 @@ def test_slabs_equal_one_domain(B, oracle, n_slabs):
     for s in runner.slabs:
         s.close()
     one.close()
+
+
+# ------------------------------------------------------------------ round-2 rows on the coupled / viscous scenes, edge cases
+
+@pytest.mark.parametrize("variant", ["pcisph", "warm"])
+def test_round2_solvers_with_rigid_coupling(B, oracle, variant):
+    """PCISPH and warm-started DFSPH on config 2 at half scale with fluid-body contact: Eq. 14 reactions (accumulated over
+    every C-pass, the warm-start one included), body states and the fluid fields against the oracle."""
+    over = dict(warm_start=1, warm_start_factor=0.5) if variant == "warm" else {}
+    sc = scenes.rigid_coupling(scale=0.5, seed=0, steps=12, **over)
+    g, o = make_pair(sc, oracle)
+    v0 = torch.zeros((g.nf, 3), dtype=torch.float32, device="cuda"); v0[:, 2] = -3.0
+    g.sph_write_state(B.VEL, v0)
+    p0 = g.sph_read_state(B.POS).clone(); p0[:, 2] -= 0.18
+    g.sph_write_state(B.POS, p0)
+    method = "pcisph" if variant == "pcisph" else "dfsph"
+    for k in range(10):
+        e, st = resync_step(g, o, sc, method=method, dv_floor_per_pass=2.5e-5)
+        check_errors(e, sc)
+        fg = np_(g.sph_read_state(B.BOUNDARY_FORCE)).astype(np.float64)
+        fo = o.boundary_force()
+        if np.abs(fo).max() > 0:
+            assert np.abs(fg - fo).max() <= TOL * np.abs(fo).max() + 1e-9
+        for bg, bo in zip(g.read_bodies(), o.bodies()):
+            check_body_state(bg, bo, sc, k)
+    assert np.abs(o.boundary_force()).max() > 0, "the test must exercise the coupling"
+    g.close(); o.close()
+
+
+def test_warm_start_with_explicit_viscosity_and_graph_equivalence(B, oracle):
+    """Warm start on the viscous config-1 scene at reduced size (the density solve then works on the viscosity kernel's
+    output records), and graph == host-driven launches bit for bit with warm start on."""
+    kw = dict(viscosity_mode=1, kinematic_viscosity=0.01, warm_start=1, warm_start_factor=0.5, eta_density=1e-4)
+    sc = scenes.dam_break((24, 24, 24), (48, 24, 24), steps=30, **kw)
+    g, o = make_pair(sc, oracle)
+    g.sph_step_dfsph(25)
+    e, st = resync_step(g, o, sc, dv_floor_per_pass=2.5e-5)
+    check_errors(e, sc)
+    g.close(); o.close()
+    outs = []
+    for over in (dict(), dict(use_cuda_graph=0)):
+        s = B.Sim.from_scene(sc, **over)
+        s.sph_step_dfsph(20)
+        outs.append((np_(s.sph_read_state(B.POS)), np_(s.sph_read_state(B.KSUM_DENSITY)), s.sph_read_stats()["total_it_d"]))
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1]) and outs[0][2] == outs[1][2]
+
+
+def test_surface_and_slab_edge_cases(B, oracle):
+    """No fluid inside the surface grid -> zero triangles, zero field; a grid that sticks out of the simulation domain
+    still gives the right field on its inside nodes; slab calls refuse a simulation that launches CUDA graphs."""
+    from oracle import surface_ref as SR
+    sc = scenes.config(0)
+    g = B.Sim.from_scene(sc)
+    g.sph_build_grid()
+    h = sc.params["support_radius"]
+    phi, tris, n = g.sph_surface_extract((0.30, 0.30, 0.45), (8, 8, 4), 0.01)      # above the block, inside the tank
+    assert n == 0 and len(tris) == 0 and float(phi.abs().max()) == 0.0
+    gmin, dims, cs = (-0.3, -0.3, 0.1), (40, 40, 6), 0.02                        # starts far outside the domain
+    phi, tris, n = g.sph_surface_extract(gmin, dims, cs)
+    pos = np_(g.sph_read_state(B.POS)).astype(np.float64)
+    rho = np_(g.sph_read_state(B.DENSITY)).astype(np.float64)
+    ref = SR.scalar_field(pos, sc.params["rest_density"] * (2 * sc.params["particle_radius"]) ** 3 / rho, h, gmin, dims, cs)
+    assert np.abs(np_(phi) - ref).max() <= 2e-5 and ref.max() > 0.5 and n > 0
+    with pytest.raises(B.SphError):
+        g.sph_slab_phase(0)
+    g.close()
