@@ -458,7 +458,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": W, "ms_per_step": 1e3 * dt / K, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": full.name, "sample_n_fluid": sc.n_fluid, "solver": "DFSPH"},
+        "config": {"workload": full.name, "n_fluid": full.n_fluid, "n_boundary": full.n_boundary, "dt": full.params["dt"],
+                   "solver": "DFSPH", "sample_n_fluid": sc.n_fluid},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": sphref.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))

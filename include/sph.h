@@ -254,7 +254,7 @@ int sph_slab_set_loop(SphSim *sim, int mode, int cont, int it, float err);
 int sph_slab_store(SphSim *sim, const float **pos4, const float **vel4, const int **orig_idx, int *n, int *n_owned);
 /* Deterministic selection (input order kept) of the entries i < n with x_lo <= pos4[i].x < x_hi and, when key != NULL,
  * key[i] < key_lt: copies pos4 / vel4, the id gid[key ? key[i] : i] and (optionally) i itself.  All arrays DEVICE except
- * count_host; scratch: >= n + 8 + (n + 1) / 4096 ints.  Synchronises the stream.  Not tied to a simulation. */
+ * count_host; scratch: 16-byte aligned, >= n + 8 + (n + 1) / 4096 ints.  Synchronises the stream.  Not tied to a simulation. */
 int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, const int *gid, const int *key, int key_lt,
                      int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
                      int max_out, int *scratch, size_t scratch_ints, int *count_host);

@@ -1090,7 +1090,7 @@ int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, co
                      int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
                      int max_out, int *scratch, size_t scratch_ints, int *count_host)
 {
-    if (n < 0 || max_out < 0 || !scratch || !count_host) return SPH_EINVAL;
+    if (n < 0 || max_out < 0 || !scratch || !count_host || (reinterpret_cast<uintptr_t>(scratch) & 15) != 0) return SPH_EINVAL;
     *count_host = 0;
     if (n == 0) return SPH_OK;
     if (!pos4 || !vel4 || !gid || (max_out > 0 && (!out_pos4 || !out_vel4 || !out_gid))) return SPH_EINVAL;
