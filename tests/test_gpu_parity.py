@@ -1112,3 +1112,34 @@ def test_surface_and_slab_edge_cases(B, oracle):
     with pytest.raises(B.SphError):
         g.sph_slab_phase(0)
     g.close()
+
+
+def test_round2_solvers_with_adaptive_dt_and_interleaved_methods(B, oracle):
+    """PCISPH and warm-started DFSPH under the CFL-adaptive time step (delta = k / dt^2 and the warm-start impulse follow
+    the step's dt), and the three step methods interleaved on one simulation (one captured graph per method), each
+    step against the oracle from the same state."""
+    kw = dict(cfl_factor=0.05, dt_min=1e-5)            # 0.05 * 2r / |v| ~ 5e-4 s < the configured 1e-3 s
+    sc = scenes.dam_break((16, 16, 24), (24, 16, 28), dt=1e-3, v0=(1.5, 0.0, -1.0), **kw)
+    g, o = make_pair(sc, oracle)
+    g.sph_step_pcisph(12)
+    for _ in range(2):
+        e, st = resync_step(g, o, sc, method="pcisph", dv_floor_per_pass=2.5e-5)
+        check_errors(e, sc)
+        assert st["dt_last"] < 1e-3                      # the CFL rule is active
+    g.close(); o.close()
+    scw = scenes.dam_break((16, 16, 24), (24, 16, 28), dt=1e-3, v0=(1.5, 0.0, -1.0), warm_start=1, warm_start_factor=0.5,
+                           eta_density=1e-4, **kw)
+    g, o = make_pair(scw, oracle)
+    g.sph_step_dfsph(12)
+    for _ in range(2):
+        e, st = resync_step(g, o, scw, dv_floor_per_pass=2.5e-5)
+        check_errors(e, scw)
+        assert st["dt_last"] < 1e-3
+    g.close(); o.close()
+    sc = scenes.dam_break((16, 16, 24), (24, 16, 28), dt=2e-4)
+    g, o = make_pair(sc, oracle)
+    for method in ("dfsph", "pcisph", "wcsph", "pcisph", "dfsph", "wcsph", "dfsph"):
+        e, st = resync_step(g, o, sc, method=method, dv_floor_per_pass=2.5e-5)
+        check_errors(e, sc)
+    assert g.sph_read_stats()["steps_done"] == 7
+    g.close(); o.close()
