@@ -266,7 +266,13 @@ int sph_set_forced_iterations(SphSim *sim, int forced_v, int forced_d, int force
 
 /* Copy one field out (un-permuted to original id order) / in.  `bytes` must equal the field's
  * size.  is_host = 0: dst/src is a device pointer, copy is asynchronous on the stream;
- * is_host = 1: host pointer, the call returns after the copy has completed.
+ * is_host = 1: host pointer, the call returns after the copy has completed;
+ * is_host = 2: PINNED host pointer, asynchronous: the buffer must stay valid and untouched until sph_host_sync()
+ *              returns.  Reads run on the simulation's stream.  Writes (fluid fields only) run on a second, internal
+ *              stream: a write starts after everything enqueued before it (steps, and earlier asynchronous reads that
+ *              may still be filling `src`) and overlaps what is enqueued after it, until a call needs the written array
+ *              (a step, sph_build_grid, a read of the same array), which waits for it.  PCIe is full duplex: the upload of
+ *              the next step's positions can run beside the download of this step's velocities.
  * sph_write_state (any writable field) invalidates grid-derived fields until the next
  * sph_build_grid / step.  Boundary fields take effect at that next sph_build_grid / step call (or at the next
  * sph_read_state of a boundary / body field, which then already shows the re-posed samples):
@@ -281,6 +287,9 @@ int sph_set_forced_iterations(SphSim *sim, int forced_v, int forced_d, int force
  *                            first_particle / n_particles / dynamic must not change. */
 int sph_read_state(SphSim *sim, int field, void *dst, size_t bytes, int is_host);
 int sph_write_state(SphSim *sim, int field, const void *src, size_t bytes, int is_host);
+
+/* Waits for everything enqueued for this simulation, asynchronous host copies included. */
+int sph_host_sync(SphSim *sim);
 
 /* The only call that always synchronises: copies the device statistics block to the host. */
 int sph_read_stats(SphSim *sim, SphStats *dst_host);

@@ -25,7 +25,7 @@ SPH_OK, SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA, SPH_EDOMAIN, SPH_ESTATE = 0, -1, -2, 
 
 EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid", "sph_step_dfsph",
            "sph_step_wcsph", "sph_step_pcisph", "sph_set_forced_iterations", "sph_read_state", "sph_write_state",
-           "sph_read_stats", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
+           "sph_read_stats", "sph_host_sync", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
            "sph_surface_workspace_bytes", "sph_surface_extract", "sph_slab_set_particles", "sph_slab_phase",
            "sph_slab_gather", "sph_slab_scatter", "sph_slab_read_error_sum", "sph_slab_set_loop", "sph_slab_store",
            "sph_select_range", "sph_last_error", "sph_destroy"]
@@ -116,6 +116,7 @@ def load() -> C.CDLL:
         L.sph_read_state.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_int]
         L.sph_write_state.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_int]
         L.sph_read_stats.argtypes = [C.c_void_p, C.POINTER(SphStats)]
+        L.sph_host_sync.argtypes = [C.c_void_p]
         L.sph_launch_count.restype = C.c_longlong
         L.sph_launch_count.argtypes = [C.c_void_p]
         L.sph_enable_kernel_timing.argtypes = [C.c_void_p, C.c_int]
@@ -310,6 +311,23 @@ class Sim:
         nbytes = out.numel() * out.element_size()
         self._check(load().sph_read_state(self._h, field, C.c_void_p(out.data_ptr()), nbytes, 1))
         return out
+
+    def sph_read_state_host_async(self, field: int, out):
+        """Asynchronous host read into a PINNED CPU tensor (is_host = 2): valid after sph_host_sync()."""
+        assert out.is_pinned()
+        nbytes = out.numel() * out.element_size()
+        self._check(load().sph_read_state(self._h, field, C.c_void_p(out.data_ptr()), nbytes, 2))
+        return out
+
+    def sph_write_state_host_async(self, field: int, src):
+        """Asynchronous host write from a PINNED CPU tensor (is_host = 2); the tensor must stay untouched until
+        sph_host_sync() or the next step has consumed it."""
+        assert src.is_pinned() and src.is_contiguous()
+        nbytes = src.numel() * src.element_size()
+        self._check(load().sph_write_state(self._h, field, C.c_void_p(src.data_ptr()), nbytes, 2))
+
+    def sph_host_sync(self):
+        self._check(load().sph_host_sync(self._h))
 
     def sph_write_state(self, field: int, src):
         t = self._torch

@@ -77,8 +77,11 @@ struct SphSim {
     SphRigidBody *bodies = nullptr;
     DevControl *ctl = nullptr;
     DevStats *stats = nullptr;
-    void *staging = nullptr;
+    void *staging = nullptr, *staging_in = nullptr;   // device staging of host reads / of asynchronous host writes
     size_t staging_bytes = 0;
+    cudaStream_t copy_stream = nullptr;   // asynchronous host writes (is_host = 2) run here, beside reads on the main stream
+    cudaEvent_t ev_main = nullptr, ev_write = nullptr;
+    unsigned pending_writes = 0;    // arrays with an asynchronous write in flight (WR_* bits)
     // host
     int *pinned = nullptr;          // small pinned block (loop predicate, stats)
     int boundary_dirty = 0;         // DIRTY_* bits: boundary fields written through sph_write_state since the last refresh
@@ -152,6 +155,27 @@ int upload(SphSim *s, void *dst_dev, const void *src_host, size_t bytes)
 }
 
 inline int cdiv(long long a, int b) { return (int)((a + b - 1) / b); }
+
+// Asynchronous host writes (sph_write_state, is_host = 2) run on a second stream so that the upload of one field can
+// overlap the download of another (PCIe is full duplex).  WR_*: which persistent arrays a pending write touches.
+enum { WR_POS = 1, WR_VEL = 2, WR_BOUNDARY = 4 };
+unsigned write_mask(int field)
+{
+    switch (field) {
+    case SPH_FIELD_POS: case SPH_FIELD_KSUM_DENSITY: return WR_POS;
+    case SPH_FIELD_VEL: case SPH_FIELD_KSUM_DIVERGENCE: return WR_VEL;
+    default: return WR_BOUNDARY | WR_POS | WR_VEL;
+    }
+}
+// everything enqueued on the main stream from now on sees the pending asynchronous writes
+int join_writes(SphSim *s)
+{
+    if (s->pending_writes) {
+        CUDA_TRY(s, cudaStreamWaitEvent(s->stream, s->ev_write, 0));
+        s->pending_writes = 0;
+    }
+    return SPH_OK;
+}
 
 struct DeviceGuard {
     int prev = -1;
@@ -295,6 +319,7 @@ size_t layout(SphSim &s, void *base)
     if (st < sizeof(SphRigidBody) * (size_t)(s.nbodies + 1)) st = sizeof(SphRigidBody) * (size_t)(s.nbodies + 1);
     s.staging_bytes = st;
     s.staging = w.take<char>(st);
+    s.staging_in = w.take<char>(st);
     return w.off;
 }
 
@@ -660,6 +685,7 @@ int do_steps(SphSim *s, int method, int n_steps)
     if (method == 2 && s->prm.viscosity_mode == 2) { s->err = "sph_step_pcisph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
     if (method == 1 && s->prm.viscosity_mode == 2) { s->err = "sph_step_wcsph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
     DeviceGuard dg(s->device);
+    { int rc = join_writes(s); if (rc) return rc; }
     if (n_steps > 0) { int rc = refresh_boundary(s); if (rc) return rc; }
     if (s->prm.cfl_factor > 0.f && !s->vmax_valid && n_steps > 0 && s->c.nf > 0) {
         // the CFL rule needs max |v| at the start of the step; later steps get it from the integration tail
@@ -748,9 +774,8 @@ int export_field(SphSim *s, int field, void *out, size_t bytes)
     return SPH_OK;
 }
 
-int import_field(SphSim *s, int field, const void *src, size_t bytes)
+int import_field(SphSim *s, int field, const void *src, size_t bytes, cudaStream_t st)
 {
-    cudaStream_t st = s->stream;
     const int nf = s->c.nf, nb = s->c.nb;
     if (bytes == 0) return SPH_OK;
     switch (field) {
@@ -806,7 +831,7 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
     s->cap = n_fluid;
     s->stream = static_cast<cudaStream_t>(cuda_stream);
     s->cur_counter = &s->misc_launches;
-    auto fail = [&](int code) { g_create_error = s->err; if (s->cap_stream) cudaStreamDestroy(s->cap_stream); if (s->pinned) cudaFreeHost(s->pinned); delete s; return code; };
+    auto fail = [&](int code) { g_create_error = s->err; if (s->cap_stream) cudaStreamDestroy(s->cap_stream); if (s->copy_stream) cudaStreamDestroy(s->copy_stream); if (s->ev_main) cudaEventDestroy(s->ev_main); if (s->ev_write) cudaEventDestroy(s->ev_write); if (s->pinned) cudaFreeHost(s->pinned); delete s; return code; };
     if (!make_const(*params, n_fluid, n_boundary, s->c, s->err)) return fail(s->err.find("grid") != std::string::npos ? SPH_EDOMAIN : SPH_EINVAL);
     if (n_fluid > 0 && (!buf->fluid_pos || !buf->fluid_vel)) { s->err = "fluid_pos / fluid_vel is NULL"; return fail(SPH_EINVAL); }
     if (n_boundary > 0 && (!buf->boundary_pos || !buf->boundary_body)) { s->err = "boundary_pos / boundary_body is NULL"; return fail(SPH_EINVAL); }
@@ -836,6 +861,9 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
     auto run = [&]() -> int {
         cudaStream_t st = s->stream;
         CUDA_TRY(s, cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+        CUDA_TRY(s, cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+        CUDA_TRY(s, cudaEventCreateWithFlags(&s->ev_main, cudaEventDisableTiming));
+        CUDA_TRY(s, cudaEventCreateWithFlags(&s->ev_write, cudaEventDisableTiming));
         CUDA_TRY(s, cudaMallocHost(&s->pinned, 4096));
         // The list passes keep only a 4.6 KB run table per CTA in shared memory and are bound by the L1
         // gather path: ask for a small shared-memory carveout so that most of the 256 KB of an SM is L1
@@ -916,6 +944,7 @@ int sph_build_grid(SphSim *s)
     if (!s) return SPH_EINVAL;
     DeviceGuard dg(s->device);
     cudaStream_t st = s->stream;
+    { int rc = join_writes(s); if (rc) return rc; }
     { int rc = refresh_boundary(s); if (rc) return rc; }
     LAUNCH(s, k_list_counters_reset, 1, 1, st, s->stats);
     if (s->c.has_dynamic) {
@@ -953,7 +982,7 @@ int slab_check(SphSim *s)
     if (s->c.has_dynamic) { s->err = "slab mode supports static boundaries only"; return SPH_ESTATE; }
     if (s->prm.viscosity_mode == 2 || s->prm.warm_start) { s->err = "slab mode: implicit viscosity and warm start are not supported"; return SPH_ESTATE; }
     if (s->prm.cfl_factor > 0.f) { s->err = "slab mode: the CFL-adaptive time step needs a global velocity maximum and is not supported"; return SPH_ESTATE; }
-    return SPH_OK;
+    return join_writes(s);
 }
 template <bool LIST>
 int slab_phase_t(SphSim *s, int phase)
@@ -1132,12 +1161,15 @@ int sph_read_state(SphSim *s, int field, void *dst, size_t bytes, int is_host)
     if (fi.derived && !s->derived_valid) { s->err = "field is stale: call sph_build_grid or a step first"; return SPH_ESTATE; }
     DeviceGuard dg(s->device);
     // pending boundary / body writes become visible to reads as well (samples re-posed, Psi recomputed)
+    // a pending asynchronous write of an array this read touches has to land first (reads of other arrays overlap it)
+    if (s->pending_writes & write_mask(field)) { int rc = join_writes(s); if (rc) return rc; }
     if (s->boundary_dirty && field >= SPH_FIELD_BOUNDARY_POS) { int rc = refresh_boundary(s); if (rc) return rc; }
     if (!is_host) return export_field(s, field, dst, bytes);
     if (bytes > s->staging_bytes) { s->err = "field too large for a host read; read it into a device buffer"; return SPH_EINVAL; }
     int rc = export_field(s, field, s->staging, bytes);
     if (rc) return rc;
     if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(dst, s->staging, bytes, cudaMemcpyDeviceToHost, s->stream));
+    if (is_host == 2) return SPH_OK;                   // asynchronous: the caller waits with sph_host_sync
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return SPH_OK;
 }
@@ -1151,17 +1183,42 @@ int sph_write_state(SphSim *s, int field, const void *src, size_t bytes, int is_
     if (bytes > 0 && !src) { s->err = "src is NULL"; return SPH_EINVAL; }
     DeviceGuard dg(s->device);
     int rc;
+    if (is_host == 2) {
+        // asynchronous host write on the copy stream: ordered after everything enqueued on the main stream so far
+        // (earlier steps, and earlier asynchronous READS that may be filling `src`), beside what follows there
+        if (bytes > s->staging_bytes) { s->err = "field too large for a host write"; return SPH_EINVAL; }
+        if (field >= SPH_FIELD_BOUNDARY_POS && field != SPH_FIELD_KSUM_DIVERGENCE && field != SPH_FIELD_KSUM_DENSITY) { s->err = "asynchronous host writes are for the fluid fields"; return SPH_EINVAL; }
+        CUDA_TRY(s, cudaEventRecord(s->ev_main, s->stream));
+        CUDA_TRY(s, cudaStreamWaitEvent(s->copy_stream, s->ev_main, 0));
+        if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging_in, src, bytes, cudaMemcpyHostToDevice, s->copy_stream));
+        rc = import_field(s, field, s->staging_in, bytes, s->copy_stream);
+        if (rc) return rc;
+        CUDA_TRY(s, cudaEventRecord(s->ev_write, s->copy_stream));
+        s->pending_writes |= write_mask(field);
+        s->derived_valid = false;
+        return SPH_OK;
+    }
+    if ((rc = join_writes(s))) return rc;
     if (is_host) {
         if (bytes > s->staging_bytes) { s->err = "field too large for a host write"; return SPH_EINVAL; }
         if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging, src, bytes, cudaMemcpyHostToDevice, s->stream));
-        rc = import_field(s, field, s->staging, bytes);
+        rc = import_field(s, field, s->staging, bytes, s->stream);
         if (rc) return rc;
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     } else {
-        rc = import_field(s, field, src, bytes);
+        rc = import_field(s, field, src, bytes, s->stream);
         if (rc) return rc;
     }
     s->derived_valid = false;
+    return SPH_OK;
+}
+
+int sph_host_sync(SphSim *s)
+{
+    if (!s) return SPH_EINVAL;
+    DeviceGuard dg(s->device);
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->copy_stream));
     return SPH_OK;
 }
 
@@ -1280,6 +1337,7 @@ int sph_surface_extract(SphSim *s, const SphSurfaceParams *sp, void *workspace, 
     if (!s->derived_valid) { s->err = "the surface is extracted from the sorted store of the last sph_build_grid / step: call sph_build_grid first"; return SPH_ESTATE; }
     DeviceGuard dg(s->device);
     cudaStream_t st = s->stream;
+    { int rc = join_writes(s); if (rc) return rc; }
     if (s->device >= 0 && s->device < 64 && !g_mc_table_ready[s->device]) {
         unsigned char cnt[256], edg[256 * kMcMaxTris * 3];
         memset(edg, 0, sizeof edg);
@@ -1317,6 +1375,9 @@ void sph_destroy(SphSim *s)
     if (!s) return;
     DeviceGuard dg(s->device);
     cudaStreamSynchronize(s->stream);
+    if (s->copy_stream) { cudaStreamSynchronize(s->copy_stream); cudaStreamDestroy(s->copy_stream); }
+    if (s->ev_main) cudaEventDestroy(s->ev_main);
+    if (s->ev_write) cudaEventDestroy(s->ev_write);
     for (int m = 0; m < 3; ++m) if (s->exec[m]) cudaGraphExecDestroy(s->exec[m]);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     if (s->pinned) cudaFreeHost(s->pinned);

@@ -1143,3 +1143,36 @@ def test_round2_solvers_with_adaptive_dt_and_interleaved_methods(B, oracle):
         check_errors(e, sc)
     assert g.sph_read_stats()["steps_done"] == 7
     g.close(); o.close()
+
+
+def test_asynchronous_host_copies(B, oracle):
+    """is_host = 2 (include/sph.h): asynchronous reads into / writes from pinned host memory.  The pipelined loop of
+    bench.py's end-to-end leg (step, read x, write x, read v, write v, all asynchronous) gives bit-identical states to
+    the same loop with synchronous copies and to free-running steps; a read of an array with a pending write sees the
+    written data."""
+    sc = scenes.splash(n_target=3e4)
+    a, b, c = (B.Sim.from_scene(sc) for _ in range(3))
+    nf = a.nf
+    ph = torch.empty((nf, 3), dtype=torch.float32).pin_memory(); vh = torch.empty((nf, 3), dtype=torch.float32).pin_memory()
+    ps = torch.empty((nf, 3), dtype=torch.float32).pin_memory(); vs = torch.empty((nf, 3), dtype=torch.float32).pin_memory()
+    for _ in range(6):
+        a.sph_step_dfsph(1)
+        a.sph_read_state_host_async(B.POS, ph); a.sph_write_state_host_async(B.POS, ph)
+        a.sph_read_state_host_async(B.VEL, vh); a.sph_write_state_host_async(B.VEL, vh)
+        b.sph_step_dfsph(1)
+        b.sph_read_state_host(B.POS, ps); b.sph_read_state_host(B.VEL, vs)
+        b.sph_write_state(B.POS, ps); b.sph_write_state(B.VEL, vs)
+    a.sph_host_sync()
+    c.sph_step_dfsph(6)
+    for fld in (B.POS, B.VEL):
+        assert torch.equal(a.sph_read_state(fld), b.sph_read_state(fld))
+        assert torch.equal(a.sph_read_state(fld), c.sph_read_state(fld))
+    assert torch.equal(ph, ps) and torch.equal(vh, vs)
+    # a pending write is visible to a later read of the same array
+    ph.mul_(0.5)
+    a.sph_write_state_host_async(B.POS, ph)
+    got = a.sph_read_state(B.POS)
+    a.sph_host_sync()
+    assert torch.equal(got.cpu(), ph)
+    for s in (a, b, c):
+        s.close()
