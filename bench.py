@@ -208,9 +208,15 @@ def run_ours(args):
         sc = scenes.splash(n_target=args.n_target, seed=rank, name="config4_splash_sweep_%.3gM" % (args.n_target / 1e6))
     else:
         sc = scenes.config(args.config, seed=rank)
+    if args.warm_start:
+        sc.params.update(warm_start=1, warm_start_factor=0.5)
+    if args.eta_density:
+        sc.params["eta_density"] = args.eta_density
     K, W = args.steps, args.warmup
     sim = B.Sim.from_scene(sc, device=local_rank, use_cuda_graph=0 if args.no_graph else 1)
     stream = sim.stream
+    step_of = lambda s_: {"dfsph": s_.sph_step_dfsph, "pcisph": s_.sph_step_pcisph, "wcsph": s_.sph_step_wcsph}[args.method]
+    sim_step = step_of(sim)
 
     def barrier():
         if world > 1:
@@ -218,7 +224,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps
-    sim.sph_step_dfsph(W)
+    sim_step(W)
     launches0 = sim.sph_launch_count()
     st0 = sim.sph_read_stats()
     clocks = ClockSampler(local_rank)
@@ -226,7 +232,7 @@ def run_ours(args):
     clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    sim.sph_step_dfsph(K)
+    sim_step(K)
     e1.record(stream)
     stream.synchronize()
     barrier()
@@ -250,7 +256,7 @@ def run_ours(args):
     sim.sph_read_state_host(B.POS, ph); sim.sph_read_state_host(B.VEL, vh)
 
     def e2e_step():
-        sim.sph_step_dfsph(1)
+        sim_step(1)
         sim.sph_read_state_host_async(B.POS, ph)
         sim.sph_write_state_host_async(B.POS, ph)
         sim.sph_read_state_host_async(B.VEL, vh)
@@ -281,12 +287,12 @@ def run_ours(args):
         done = int(sim.sph_read_stats()["steps_done"])
         first = max(done, args.impact_first_step)
         if first > done:
-            sim.sph_step_dfsph(first - done)
+            sim_step(first - done)
         Ki = max(1, min(K, 30))
         stA = sim.sph_read_stats()
         barrier()
         e0.record(stream)
-        sim.sph_step_dfsph(Ki)
+        sim_step(Ki)
         e1.record(stream)
         stream.synchronize()
         barrier()
@@ -306,7 +312,9 @@ def run_ours(args):
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": sc.name, "n_fluid": nf, "n_boundary": sc.n_boundary,
-                       "n_cells": int(sim.ncells), "dt": sc.params["dt"], "solver": "DFSPH",
+                       "n_cells": int(sim.ncells), "dt": sc.params["dt"],
+                       "solver": {"dfsph": "DFSPH", "pcisph": "PCISPH", "wcsph": "WCSPH"}[args.method] + (" + warm start" if args.warm_start else ""),
+                       "eta_density": sc.params["eta_density"],
                        "mean_it_v": mean_it_v, "mean_it_d": mean_it_d,
                        "neighbour_passes_per_step": 1 + 2 * mean_it_v + 2 * mean_it_d,
                        "parallelism": "replicas x%d" % world if world > 1 else "1 GPU",
@@ -326,7 +334,7 @@ def run_ours(args):
     # cannot bracket nodes inside a graph's WHILE body), rank 0 only -> roofline of the dominant kernel
     if rank == 0 and not args.no_breakdown:
         sim2 = B.Sim.from_scene(sc, device=local_rank, use_cuda_graph=0)
-        sim2.sph_step_dfsph(W)
+        step_of(sim2)(W)
         sim2.sph_build_grid()   # no-op for the physics: refreshes lists for the statistics below
         cnt = sim2.sph_read_state(B.NEIGHBOR_COUNT).to(torch.float64)
         nf_mean, nb_mean = float(cnt[:, 0].mean()), float(cnt[:, 1].mean())
@@ -336,7 +344,7 @@ def run_ours(args):
         box = 27.0 * torch.nn.functional.avg_pool3d(occ, 3, stride=1, padding=1, count_include_pad=True)
         cand_mean = float((occ * box).sum() / max(float(occ.sum()), 1.0)) * (2.0 + 1.0 / FINE_X) / 3.0
         sim2.sph_enable_kernel_timing(True)
-        sim2.sph_step_dfsph(K)
+        step_of(sim2)(K)
         kt = sim2.sph_read_kernel_times()
         sim2_ncells = sim2.ncells
         sim2.close()
@@ -493,6 +501,10 @@ def main():
     ap.add_argument("--no-impact-window", action="store_true")
     ap.add_argument("--impact-first-step", type=int, default=130)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--method", default="dfsph", choices=["dfsph", "pcisph", "wcsph"],
+                    help="step method (the headline metric is DFSPH; the others are the library's other solvers on the same scene)")
+    ap.add_argument("--warm-start", action="store_true", help="DFSPH with warm start (reading R27); not the headline line")
+    ap.add_argument("--eta-density", type=float, default=0.0, help="override the density tolerance (0: the config's 1e-3)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
