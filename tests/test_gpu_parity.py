@@ -1176,3 +1176,34 @@ def test_asynchronous_host_copies(B, oracle):
     assert torch.equal(got.cpu(), ph)
     for s in (a, b, c):
         s.close()
+
+
+def test_slab_runner_with_nccl_exchange_world_of_one(B, oracle):
+    """The torch.distributed exchange back end on NCCL (the multi-GPU configuration) with the one rank this box has:
+    the all-reduces of the loop control run through NCCL on the simulation's stream; one slab, no neighbours -> the
+    result equals the ordinary simulation's within the 1e-4 bar and the iteration counts agree.  (Two ranks need two
+    GPUs: the send / recv pairing is covered by the gloo test in test_multirank.py.)"""
+    import os
+    import socket
+    import torch.distributed as dist
+    from paper_2403_11156_b200 import slabs as S
+    with socket.socket() as s_:
+        s_.bind(("127.0.0.1", 0)); port = s_.getsockname()[1]
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1,
+                            device_id=torch.device("cuda", 0))
+    try:
+        sc = scenes.splash(n_target=6e4)
+        slab = S.GpuSlab(sc, -3.0e38, 3.0e38, sc.n_fluid + 4096, 4096)
+        runner = S.SlabRunner([slab], S.DistExchange(torch.device("cuda", 0)), sc.params)
+        runner.run(8)
+        one = B.Sim.from_scene(sc)
+        one.sph_step_dfsph(8)
+        st = one.sph_read_stats()
+        assert (runner.stats["total_it_v"], runner.stats["total_it_d"]) == (st["total_it_v"], st["total_it_d"])
+        g_, p_, v_ = slab.owned_state()
+        vel = np_(one.sph_read_state(B.VEL)).astype(np.float64)
+        assert np.linalg.norm(v_ - vel[g_], axis=1).max() <= 1e-4 * np.linalg.norm(vel, axis=1).max()
+        assert len(g_) == sc.n_fluid
+        slab.close(); one.close()
+    finally:
+        dist.destroy_process_group()
