@@ -1207,3 +1207,26 @@ def test_slab_runner_with_nccl_exchange_world_of_one(B, oracle):
         slab.close(); one.close()
     finally:
         dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("variant", ["pcisph", "warm"])
+def test_round2_solvers_full_size_config4(B, oracle, variant):
+    """The round-2 solvers at the headline size (config 4, 1.23M particles) on the post-impact state: 100 free-running
+    steps, then two resynchronised steps against the oracle (rho, alpha, v, x within 1e-4; for the warm-started run
+    under a tight tolerance, so that the loops run above their minimum and the stored totals matter)."""
+    over = dict(warm_start=1, warm_start_factor=0.5, eta_density=1e-5) if variant == "warm" else {}
+    sc = scenes.config(4, **over)
+    g, o = make_pair(sc, oracle)
+    method = "pcisph" if variant == "pcisph" else "dfsph"
+    (g.sph_step_pcisph if variant == "pcisph" else g.sph_step_dfsph)(100)
+    its = []
+    for _ in range(2):
+        e, st = resync_step(g, o, sc, method=method, dv_floor_per_pass=2.5e-5)
+        check_errors(e, sc)
+        assert st["overflow_count"] == 0 and st["nan_count"] == 0 and st["max_iter_hit"] == 0
+        its.append(st["it_d"])
+    assert min(its) >= 3 if variant == "pcisph" else max(its) >= 2
+    if variant == "warm":
+        kd = np_(g.sph_read_state(B.KSUM_DENSITY)).astype(np.float64)
+        assert np.abs(kd - o.ksum_d()).max() <= 1e-4 * np.abs(o.ksum_d()).max() and kd.max() > 0
+    g.close(); o.close()
