@@ -206,6 +206,9 @@ __device__ __noinline__ void spill_walk(const PassCtx &p, const float *__restric
             }
         }
     }
+    // the passes decode both halves of a list word without a guard: the unwritten half of an odd tail pair must be a
+    // decodable entry (the copy-out zeroes it for staged entries; here the pair may lie past the staged rows)
+    if (k > rows && (k & 1) && k < p.c.kf) gl[(size_t)(k >> 1) * 64 + 1] = 0;
 }
 
 __global__ void __launch_bounds__(32 * kBuildWarps, 8)

@@ -166,11 +166,13 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
             for (int t = 0; t < PB; ++t) nxt[t] = pb + PB + t < npair ? ldg_stream(lp + (pb + PB + t) * 32) : 0u;
             int jj[2 * PB];
             float4 q[2 * PB], q2[NSRC >= 2 ? 2 * PB : 1];
+            const int rem = cf - 2 * pb;                  // entries left, this stage included
 #pragma unroll
             for (int u = 0; u < 2 * PB; ++u) {
-                const bool valid = 2 * pb + u < cf;
-                uint32_t e = (u & 1) ? (cur[u >> 1] >> 16) : (cur[u >> 1] & 0xffffu);
-                e = valid ? e : 0u;                       // the unwritten half of an odd tail pair is garbage
+                const bool valid = u < rem;
+                // (words past the list are 0 and the builder zeroes the unwritten half of an odd tail pair: every
+                // slot decodes to a table entry, no guard needed before the look-up)
+                const uint32_t e = (u & 1) ? (cur[u >> 1] >> 16) : (cur[u >> 1] & 0xffffu);
                 int j = tbl[(e >> kOffBits) * kBlock] + (int)(e & kOffMask);
                 jj[u] = valid ? j : i;
                 // predicated record gather: a lane whose list has ended issues no memory access at all (its registers
@@ -184,7 +186,7 @@ __device__ __forceinline__ void for_each_neighbor(const PassCtx &p, const float4
             }
 #pragma unroll
             for (int u = 0; u < 2 * PB; ++u) {
-                if ((PADSAFE && NSRC != 3) || 2 * pb + u < cf) {
+                if ((PADSAFE && NSRC != 3) || u < rem) {
                     float dx = __fsub_rn(xi, q[u].x), dy = __fsub_rn(yi, q[u].y), dz = __fsub_rn(zi, q[u].z);
                     ff(jj[u], q[u], NSRC >= 2 ? q2[u] : q[u], dx, dy, dz, dist2_r10(dx, dy, dz));
                 }
