@@ -1047,6 +1047,33 @@ def test_slabs_equal_one_domain(B, oracle, n_slabs):
     one.close()
 
 
+def test_slabs_with_explicit_viscosity_equal_one_domain(B, oracle):
+    """Slab mode with the Eq. 15 kernel in the step (the velocity refresh after the viscosity pass, the record array
+    that the density solve then works on): the viscous dam break of config 1 at reduced size in two slabs, cut inside
+    the block, against the single domain over 15 steps."""
+    from paper_2403_11156_b200 import slabs as S
+    sc = scenes.dam_break((24, 24, 24), (48, 24, 24), steps=15, viscosity_mode=1, kinematic_viscosity=0.01)
+    one = B.Sim.from_scene(sc)
+    runner, cuts = S.make_local_slabs(sc, 2)
+    runner.run(15)
+    one.sph_step_dfsph(15)
+    st = one.sph_read_stats()
+    assert (runner.stats["total_it_v"], runner.stats["total_it_d"]) == (st["total_it_v"], st["total_it_d"])
+    pos, vel = np_(one.sph_read_state(B.POS)).astype(np.float64), np_(one.sph_read_state(B.VEL)).astype(np.float64)
+    vscale = max(np.linalg.norm(vel, axis=1).max(), np.sqrt(9.81 * 24 * 2 * sc.params["particle_radius"]))
+    seen = np.zeros(sc.n_fluid, dtype=int)
+    for s in runner.slabs:
+        assert s.n_total > s.n_owned
+        g, p_, v_ = s.owned_state()
+        seen[g] += 1
+        assert np.linalg.norm(v_ - vel[g], axis=1).max() <= 1e-4 * vscale
+        assert np.abs(p_ - pos[g]).max() <= 15 * sc.params["dt"] * 1e-4 * vscale + 1e-6
+    assert (seen == 1).all()
+    for s in runner.slabs:
+        s.close()
+    one.close()
+
+
 # ------------------------------------------------------------------ round-2 rows on the coupled / viscous scenes, edge cases
 
 @pytest.mark.parametrize("variant", ["pcisph", "warm"])
