@@ -335,10 +335,10 @@ int enqueue_grid(SphSim *s, cudaStream_t st, GridBufs &g, const float4 *a_in, co
     LAUNCH(s, k_scan_tile_sums, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
     LAUNCH(s, k_scan_apply, g.ntiles, kScanThreads, st, g.cell_start, nscan, g.tile_sum);
     if (g.n > 0) {
-        LAUNCH(s, k_scatter_slots, cdiv(g.n, 256), 256, st, g.key, g.off, g.cell_start, g.n, g.slot);
-        if (fluid) LAUNCH(s, k_reorder<true>, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
+        LAUNCH(s, k_scatter_slots, cdiv(g.n, 256 * kScatterPer), 256, st, g.key, g.off, g.cell_start, g.n, g.slot);
+        if (fluid) LAUNCH(s, k_reorder<true>, cdiv(g.n, 256 * kReorderPer), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
                           a_out, b_out, id_out, s->px, s->py, s->pz);
-        else       LAUNCH(s, k_reorder<false>, cdiv(g.n, 256), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
+        else       LAUNCH(s, k_reorder<false>, cdiv(g.n, 256 * kReorderPer), 256, st, g.slot, g.key, g.cell_start, g.n, a_in, b_in, id_in,
                           a_out, b_out, id_out, (float *)nullptr, (float *)nullptr, (float *)nullptr);
     }
     return SPH_OK;
