@@ -81,6 +81,11 @@ struct SphSim {
     size_t staging_bytes = 0;
     cudaStream_t copy_stream = nullptr;   // asynchronous host writes (is_host = 2) run here, beside reads on the main stream
     cudaEvent_t ev_main = nullptr, ev_write = nullptr;
+    // chunk-wise pipelining of an asynchronous host read with the asynchronous write that uploads the same buffer again
+    static constexpr int kHostChunks = 4;
+    cudaEvent_t ev_chunk[kHostChunks] = {};
+    unsigned long long op_seq = 0;                 // bumped by every API call that may enqueue work on the main stream
+    struct { const void *dst = nullptr; size_t bytes = 0; unsigned long long seq = 0; } last_read;   // last asynchronous host read
     unsigned pending_writes = 0;    // arrays with an asynchronous write in flight (WR_* bits)
     // host
     int *pinned = nullptr;          // small pinned block (loop predicate, stats)
@@ -167,6 +172,11 @@ unsigned write_mask(int field)
     default: return WR_BOUNDARY | WR_POS | WR_VEL;
     }
 }
+inline size_t host_chunk_bytes(size_t bytes)
+{
+    const size_t c = (bytes + SphSim::kHostChunks - 1) / SphSim::kHostChunks;
+    return (c + 255) & ~size_t(255);
+}
 // everything enqueued on the main stream from now on sees the pending asynchronous writes
 int join_writes(SphSim *s)
 {
@@ -180,6 +190,7 @@ int join_writes(SphSim *s)
 struct DeviceGuard {
     int prev = -1;
     explicit DeviceGuard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    explicit DeviceGuard(SphSim *s) : DeviceGuard(s->device) { ++s->op_seq; }
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
@@ -544,7 +555,9 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
     const int nf = s->c.nf;
     const bool dyn = s->c.has_dynamic != 0;
     long long *bc = s->body_nodes[method];
-    LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl, s->prm.cfl_factor * 2.0f * s->prm.particle_radius, s->prm.dt_min, s->prm.dt);
+    // DFSPH / PCISPH steps with particles end in a solver loop whose last P-pass also closes the step's statistics
+    const bool fold_end = nf > 0 && method != 1;
+    LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl, s->prm.cfl_factor * 2.0f * s->prm.particle_radius, s->prm.dt_min, s->prm.dt, fold_end ? 1 : 0);
     if (dyn) {
         int rc = enqueue_boundary_grid(s, st);
         if (rc) return rc;
@@ -646,7 +659,7 @@ int enqueue_step_t(SphSim *s, int method, bool graph_mode)
         LAUNCH(s, k_rigid_step, s->nbodies, 256, st, s->c, s->bodies, s->prm.tank_min[0], s->prm.tank_min[1],
                s->prm.tank_min[2], s->prm.tank_max[0], s->prm.tank_max[1], s->prm.tank_max[2], s->brest, s->bforce,
                s->borig_pos, s->borig_vel);
-    LAUNCH(s, k_step_end, 1, 1, st, s->stats, s->ctl);
+    if (!fold_end) LAUNCH(s, k_step_end, 1, 1, st, s->stats, s->ctl);
     return SPH_OK;
 }
 
@@ -684,7 +697,7 @@ int do_steps(SphSim *s, int method, int n_steps)
     if (n_steps < 0) { s->err = "n_steps < 0"; return SPH_EINVAL; }
     if (method == 2 && s->prm.viscosity_mode == 2) { s->err = "sph_step_pcisph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
     if (method == 1 && s->prm.viscosity_mode == 2) { s->err = "sph_step_wcsph has no implicit viscosity (viscosity_mode 2): use mode 0 or 1"; return SPH_ESTATE; }
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     { int rc = join_writes(s); if (rc) return rc; }
     if (n_steps > 0) { int rc = refresh_boundary(s); if (rc) return rc; }
     if (s->prm.cfl_factor > 0.f && !s->vmax_valid && n_steps > 0 && s->c.nf > 0) {
@@ -857,13 +870,14 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
     layout(*s, buf->workspace);
     s->c.dt_dev = &s->ctl->dt;
 
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     auto run = [&]() -> int {
         cudaStream_t st = s->stream;
         CUDA_TRY(s, cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
         CUDA_TRY(s, cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
         CUDA_TRY(s, cudaEventCreateWithFlags(&s->ev_main, cudaEventDisableTiming));
         CUDA_TRY(s, cudaEventCreateWithFlags(&s->ev_write, cudaEventDisableTiming));
+        for (int k = 0; k < SphSim::kHostChunks; ++k) CUDA_TRY(s, cudaEventCreateWithFlags(&s->ev_chunk[k], cudaEventDisableTiming));
         CUDA_TRY(s, cudaMallocHost(&s->pinned, 4096));
         // The list passes keep only a 4.6 KB run table per CTA in shared memory and are bound by the L1
         // gather path: ask for a small shared-memory carveout so that most of the 256 KB of an SM is L1
@@ -942,7 +956,7 @@ int sph_create(const SphParams *params, const SphBuffers *buf, int n_fluid, int 
 int sph_build_grid(SphSim *s)
 {
     if (!s) return SPH_EINVAL;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     cudaStream_t st = s->stream;
     { int rc = join_writes(s); if (rc) return rc; }
     { int rc = refresh_boundary(s); if (rc) return rc; }
@@ -992,7 +1006,7 @@ int slab_phase_t(SphSim *s, int phase)
     const int nf = s->c.nf;
     switch (phase) {
     case SPH_SLAB_BEGIN: {
-        LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl, s->prm.cfl_factor * 2.0f * s->prm.particle_radius, s->prm.dt_min, s->prm.dt);
+        LAUNCH(s, k_step_begin, 1, 1, st, s->stats, s->ctl, s->prm.cfl_factor * 2.0f * s->prm.particle_radius, s->prm.dt_min, s->prm.dt, 0);
         int rc = enqueue_fluid_grid_and_lists(s, st);
         if (rc) return rc;
         if (nf > 0) LAUNCH(s, k_slab_inverse, cdiv(nf, 256), 256, st, s->idB, nf, s->inv);
@@ -1029,7 +1043,7 @@ int sph_slab_set_particles(SphSim *s, const float *pos4, const float *vel4, int 
     const long long n = (long long)n_owned + n_ghost;
     if (n_owned < 0 || n_ghost < 0 || n > s->cap) { char b[160]; snprintf(b, sizeof b, "slab particle count %lld exceeds the capacity %d the simulation was created with", n, s->cap); s->err = b; return SPH_ENOMEM; }
     if (n > 0 && (!pos4 || !vel4)) { s->err = "pos4 / vel4 is NULL"; return SPH_EINVAL; }
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     cudaStream_t st = s->stream;
     s->c.nf = (int)n; s->c.nown = n_owned;
     s->gf.n = (int)n;
@@ -1051,7 +1065,7 @@ int sph_slab_phase(SphSim *s, int phase)
 {
     int rc = slab_check(s);
     if (rc) return rc;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     return s->prm.use_neighbor_list ? slab_phase_t<true>(s, phase) : slab_phase_t<false>(s, phase);
 }
 
@@ -1061,7 +1075,7 @@ int sph_slab_gather(SphSim *s, int what, const int *orig_idx, int n, float *out4
     if (rc) return rc;
     if (n < 0 || (n > 0 && (!orig_idx || !out4)) || (what != SPH_SLAB_FIELD_KR && what != SPH_SLAB_FIELD_VEL)) { s->err = "sph_slab_gather: bad argument"; return SPH_EINVAL; }
     if (n == 0) return SPH_OK;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     const float4 *f = what == SPH_SLAB_FIELD_KR ? s->posk : &s->slab_vcur->v;
     LAUNCH(s, k_slab_gather, cdiv(n, 256), 256, s->stream, f, what == SPH_SLAB_FIELD_KR ? 1 : 2, s->inv, orig_idx, n, reinterpret_cast<float4 *>(out4));
     return SPH_OK;
@@ -1073,7 +1087,7 @@ int sph_slab_scatter(SphSim *s, int what, int first_orig, int n, const float *in
     if (rc) return rc;
     if (n < 0 || first_orig < 0 || (long long)first_orig + n > s->c.nf || (n > 0 && !in4) || (what != SPH_SLAB_FIELD_KR && what != SPH_SLAB_FIELD_VEL)) { s->err = "sph_slab_scatter: bad argument"; return SPH_EINVAL; }
     if (n == 0) return SPH_OK;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     float4 *f = what == SPH_SLAB_FIELD_KR ? s->posk : &s->slab_vcur->v;
     LAUNCH(s, k_slab_scatter, cdiv(n, 256), 256, s->stream, f, what == SPH_SLAB_FIELD_KR ? 1 : 2, s->inv, first_orig, n, reinterpret_cast<const float4 *>(in4));
     return SPH_OK;
@@ -1084,7 +1098,7 @@ int sph_slab_read_error_sum(SphSim *s, unsigned long long *total)
     int rc = slab_check(s);
     if (rc) return rc;
     if (!total) return SPH_EINVAL;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     unsigned long long *h = reinterpret_cast<unsigned long long *>(s->pinned + 8);
     *h = 0ull;
     if (s->c.nf > 0) {
@@ -1099,7 +1113,7 @@ int sph_slab_set_loop(SphSim *s, int mode, int cont, int it, float err)
 {
     int rc = slab_check(s);
     if (rc) return rc;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     LAUNCH(s, k_slab_set_loop, 1, 1, s->stream, s->ctl, s->stats, mode, cont, it, err);
     return SPH_OK;
 }
@@ -1142,7 +1156,7 @@ int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, co
 int sph_set_forced_iterations(SphSim *s, int forced_v, int forced_d, int forced_cg)
 {
     if (!s) return SPH_EINVAL;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     // the three ints are the first members of DevControl
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     s->pinned[0] = forced_v; s->pinned[1] = forced_d; s->pinned[2] = forced_cg;
@@ -1159,7 +1173,7 @@ int sph_read_state(SphSim *s, int field, void *dst, size_t bytes, int is_host)
     if (bytes != fi.bytes) { char b[128]; snprintf(b, sizeof b, "field %d is %zu bytes, caller passed %zu", field, fi.bytes, bytes); s->err = b; return SPH_EINVAL; }
     if (bytes > 0 && !dst) { s->err = "dst is NULL"; return SPH_EINVAL; }
     if (fi.derived && !s->derived_valid) { s->err = "field is stale: call sph_build_grid or a step first"; return SPH_ESTATE; }
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     // pending boundary / body writes become visible to reads as well (samples re-posed, Psi recomputed)
     // a pending asynchronous write of an array this read touches has to land first (reads of other arrays overlap it)
     if (s->pending_writes & write_mask(field)) { int rc = join_writes(s); if (rc) return rc; }
@@ -1168,8 +1182,21 @@ int sph_read_state(SphSim *s, int field, void *dst, size_t bytes, int is_host)
     if (bytes > s->staging_bytes) { s->err = "field too large for a host read; read it into a device buffer"; return SPH_EINVAL; }
     int rc = export_field(s, field, s->staging, bytes);
     if (rc) return rc;
+    if (is_host == 2) {
+        // asynchronous: the caller waits with sph_host_sync.  The copy goes out in chunks with an event behind each, so
+        // that an asynchronous write of the same host buffer that follows directly can upload chunk k as soon as it has
+        // arrived (both directions of the bus busy at once), instead of after the whole field
+        CUDA_TRY(s, cudaEventRecord(s->ev_main, s->stream));           // the export kernel and all earlier work
+        const size_t chunk = host_chunk_bytes(bytes);
+        for (int k = 0; k < SphSim::kHostChunks; ++k) {
+            const size_t off = (size_t)k * chunk, len = off < bytes ? (bytes - off < chunk ? bytes - off : chunk) : 0;
+            if (len > 0) CUDA_TRY(s, cudaMemcpyAsync((char *)dst + off, s->staging + off, len, cudaMemcpyDeviceToHost, s->stream));
+            CUDA_TRY(s, cudaEventRecord(s->ev_chunk[k], s->stream));
+        }
+        s->last_read.dst = dst; s->last_read.bytes = bytes; s->last_read.seq = s->op_seq;
+        return SPH_OK;
+    }
     if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(dst, s->staging, bytes, cudaMemcpyDeviceToHost, s->stream));
-    if (is_host == 2) return SPH_OK;                   // asynchronous: the caller waits with sph_host_sync
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     return SPH_OK;
 }
@@ -1181,16 +1208,28 @@ int sph_write_state(SphSim *s, int field, const void *src, size_t bytes, int is_
     if (!field_info(s, field, fi) || !fi.writable) { s->err = "field is not writable"; return SPH_EINVAL; }
     if (bytes != fi.bytes) { char b[128]; snprintf(b, sizeof b, "field %d is %zu bytes, caller passed %zu", field, fi.bytes, bytes); s->err = b; return SPH_EINVAL; }
     if (bytes > 0 && !src) { s->err = "src is NULL"; return SPH_EINVAL; }
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     int rc;
     if (is_host == 2) {
         // asynchronous host write on the copy stream: ordered after everything enqueued on the main stream so far
         // (earlier steps, and earlier asynchronous READS that may be filling `src`), beside what follows there
         if (bytes > s->staging_bytes) { s->err = "field too large for a host write"; return SPH_EINVAL; }
         if (field >= SPH_FIELD_BOUNDARY_POS && field != SPH_FIELD_KSUM_DIVERGENCE && field != SPH_FIELD_KSUM_DENSITY) { s->err = "asynchronous host writes are for the fluid fields"; return SPH_EINVAL; }
-        CUDA_TRY(s, cudaEventRecord(s->ev_main, s->stream));
-        CUDA_TRY(s, cudaStreamWaitEvent(s->copy_stream, s->ev_main, 0));
-        if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging_in, src, bytes, cudaMemcpyHostToDevice, s->copy_stream));
+        if (bytes > 0 && src == s->last_read.dst && bytes == s->last_read.bytes && s->last_read.seq + 1 == s->op_seq) {
+            // the buffer is the target of the asynchronous read enqueued by the previous call: upload chunk k behind
+            // download chunk k (ev_main was recorded by that read, behind its export kernel and all earlier work)
+            CUDA_TRY(s, cudaStreamWaitEvent(s->copy_stream, s->ev_main, 0));
+            const size_t chunk = host_chunk_bytes(bytes);
+            for (int k = 0; k < SphSim::kHostChunks; ++k) {
+                const size_t off = (size_t)k * chunk, len = off < bytes ? (bytes - off < chunk ? bytes - off : chunk) : 0;
+                CUDA_TRY(s, cudaStreamWaitEvent(s->copy_stream, s->ev_chunk[k], 0));
+                if (len > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging_in + off, (const char *)src + off, len, cudaMemcpyHostToDevice, s->copy_stream));
+            }
+        } else {
+            CUDA_TRY(s, cudaEventRecord(s->ev_main, s->stream));
+            CUDA_TRY(s, cudaStreamWaitEvent(s->copy_stream, s->ev_main, 0));
+            if (bytes > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging_in, src, bytes, cudaMemcpyHostToDevice, s->copy_stream));
+        }
         rc = import_field(s, field, s->staging_in, bytes, s->copy_stream);
         if (rc) return rc;
         CUDA_TRY(s, cudaEventRecord(s->ev_write, s->copy_stream));
@@ -1216,7 +1255,7 @@ int sph_write_state(SphSim *s, int field, const void *src, size_t bytes, int is_
 int sph_host_sync(SphSim *s)
 {
     if (!s) return SPH_EINVAL;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     CUDA_TRY(s, cudaStreamSynchronize(s->copy_stream));
     return SPH_OK;
@@ -1225,7 +1264,7 @@ int sph_host_sync(SphSim *s)
 int sph_read_stats(SphSim *s, SphStats *o)
 {
     if (!s || !o) return SPH_EINVAL;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     DevStats *h = reinterpret_cast<DevStats *>(s->pinned + 64);
     CUDA_TRY(s, cudaMemcpyAsync(h, s->stats, sizeof(DevStats), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
@@ -1275,7 +1314,7 @@ int sph_enable_kernel_timing(SphSim *s, int enable)
 int sph_read_kernel_times(SphSim *s, char *buf, size_t bytes)
 {
     if (!s || !buf || bytes == 0) return SPH_EINVAL;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     struct Acc { std::string name; long long n; double ms; };
     std::vector<Acc> acc;
@@ -1335,7 +1374,7 @@ int sph_surface_extract(SphSim *s, const SphSurfaceParams *sp, void *workspace, 
     if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0) { s->err = "surface workspace must be 256-byte aligned"; return SPH_EINVAL; }
     if (max_triangles < 0 || (max_triangles > 0 && !triangles)) { s->err = "triangles is NULL"; return SPH_EINVAL; }
     if (!s->derived_valid) { s->err = "the surface is extracted from the sorted store of the last sph_build_grid / step: call sph_build_grid first"; return SPH_ESTATE; }
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     cudaStream_t st = s->stream;
     { int rc = join_writes(s); if (rc) return rc; }
     if (s->device >= 0 && s->device < 64 && !g_mc_table_ready[s->device]) {
@@ -1373,11 +1412,12 @@ const char *sph_last_error(const SphSim *s) { return s ? s->err.c_str() : g_crea
 void sph_destroy(SphSim *s)
 {
     if (!s) return;
-    DeviceGuard dg(s->device);
+    DeviceGuard dg(s);
     cudaStreamSynchronize(s->stream);
     if (s->copy_stream) { cudaStreamSynchronize(s->copy_stream); cudaStreamDestroy(s->copy_stream); }
     if (s->ev_main) cudaEventDestroy(s->ev_main);
     if (s->ev_write) cudaEventDestroy(s->ev_write);
+    for (int k = 0; k < SphSim::kHostChunks; ++k) if (s->ev_chunk[k]) cudaEventDestroy(s->ev_chunk[k]);
     for (int m = 0; m < 3; ++m) if (s->exec[m]) cudaGraphExecDestroy(s->exec[m]);
     if (s->cap_stream) cudaStreamDestroy(s->cap_stream);
     if (s->pinned) cudaFreeHost(s->pinned);

@@ -71,6 +71,7 @@ struct DevControl {
     float dt;                            // time step of the running step (R26; = SphParams.dt when cfl_factor = 0)
     unsigned long long acc;              // running P-pass: CTA counter (top 20 bits) | fixed-point error sum (A12)
     unsigned long long last_total;       // fixed-point error sum of the last P-pass (slab mode: summed over the slabs by the host)
+    int fold_end;                        // the P-pass that ends the step's last loop also closes the step's statistics (no k_step_end launch)
 };
 
 // Statistics block in device memory; sph_read_stats copies it out and converts to SphStats.
@@ -89,6 +90,14 @@ struct DevStats {
     float dt_last;
     double sim_time;
 };
+
+// end of a step: running totals (k_step_end, or the last CTA of the P-pass that ends the step's last solver loop)
+__device__ __forceinline__ void step_end_accumulate(DevStats *st, const DevControl *ctl)
+{
+    st->steps_done += 1;
+    st->dt_last = ctl->dt; st->sim_time += (double)ctl->dt;
+    st->total_it_v += st->it_v; st->total_it_d += st->it_d; st->total_cg += st->cg_iters;
+}
 
 // time step of the running step
 __device__ __forceinline__ float step_dt(const SimConst &c) { return __ldg(c.dt_dev); }

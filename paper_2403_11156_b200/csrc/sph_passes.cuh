@@ -289,6 +289,7 @@ __device__ __forceinline__ void solver_ctrl_eval(double err, DevControl *ctl, De
         if (MODE == MODE_DIV) { st->it_v = 0; st->err_v = 0.f; } else { st->it_d = 0; st->err_rho = 0.f; }
         ctl->it = 0;
         set_loop_condition(lh.h, lh.use_handle, ctl, 0);
+        if (MODE != MODE_DIV && ctl->fold_end) step_end_accumulate(st, ctl);
         return;
     }
     const int l = first ? 1 : ctl->it + 1;
@@ -305,6 +306,8 @@ __device__ __forceinline__ void solver_ctrl_eval(double err, DevControl *ctl, De
         cont = f > 0 ? (l < f) : ((err > (double)ctl->eta_d || l < mn) && l < mx);
         st->it_d = l; st->err_rho = (float)err;
         if (f < 0 && !cont && err > (double)ctl->eta_d) st->max_iter_hit |= 2;
+        // the density (or PCISPH pressure) loop is the step's last: its final P-pass closes the step's statistics
+        if (!cont && ctl->fold_end) step_end_accumulate(st, ctl);
     }
     set_loop_condition(lh.h, lh.use_handle, ctl, cont);
 }

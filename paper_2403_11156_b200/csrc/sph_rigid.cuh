@@ -378,8 +378,9 @@ constexpr int kCtrlThreads = 1024;   // one CTA sums the per-CTA partials: wide,
 // Start of a step: choose its dt (reading R26: dt = clamp(lambda 2r / max|v|, dt_min, dt_max) with the
 // velocities at the step's start -- st->vmax_bits holds their maximum, left there by the previous step's
 // integration or by k_vmax; cfl2r = lambda 2r, 0 = fixed dt), then reset the per-step statistics.
-__global__ void k_step_begin(DevStats *st, DevControl *ctl, float cfl2r, float dt_min, float dt_max)
+__global__ void k_step_begin(DevStats *st, DevControl *ctl, float cfl2r, float dt_min, float dt_max, int fold_end)
 {
+    ctl->fold_end = fold_end;
     float dt = dt_max;
     if (cfl2r > 0.f) {
         float vmax = __uint_as_float(st->vmax_bits);
@@ -400,9 +401,7 @@ __global__ void k_list_counters_reset(DevStats *st)
 }
 __global__ void k_step_end(DevStats *st, const DevControl *ctl)
 {
-    st->steps_done += 1;
-    st->dt_last = ctl->dt; st->sim_time += (double)ctl->dt;
-    st->total_it_v += st->it_v; st->total_it_d += st->it_d; st->total_cg += st->cg_iters;
+    step_end_accumulate(st, ctl);
 }
 
 // CG start: |b|^2, |r0|^2, first predicate (R23: stop when |r| <= tol |b| or max iterations)
