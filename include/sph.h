@@ -259,6 +259,23 @@ int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, co
                      int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
                      int max_out, int *scratch, size_t scratch_ints, int *count_host);
 
+/* sph_select_range for callers that cannot allocate device memory (code under CUDA-graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): same selection, same arguments minus the scratch -- the flag / scan scratch is a
+ * file-scope `static __device__` array inside the library, sized for n <= SPH_SELECT_STATIC_MAX entries
+ * (SPH_SELECT_STATIC_MAX + 1024 ints = 4 MiB + 4 KiB, held by every GPU that loads the library until the process exits).
+ * The call allocates nothing: no cudaMalloc / cudaFree and no allocating library routine; the array's device address is
+ * looked up once per device (cudaGetSymbolAddress, with the CURRENT device -- the one the stream and all pointers belong
+ * to -- which must be the same on every call that uses that device's array).
+ *   n > SPH_SELECT_STATIC_MAX: SPH_EINVAL, *count_host = 0, text in sph_last_error(NULL); nothing is launched.
+ *   Every call on a device shares that device's array, which keeps the last call's contents; nothing in it has to start
+ *   at zero (every word a call reads it has written itself first).  Two calls whose kernels overlap on the GPU (different
+ *   streams, or one graph launched twice concurrently) RACE on it: serialise them.  The call itself synchronises the
+ *   stream, like sph_select_range. */
+#define SPH_SELECT_STATIC_MAX (1 << 20)
+int sph_select_range_static(void *cuda_stream, const float *pos4, const float *vel4, const int *gid, const int *key, int key_lt,
+                            int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
+                            int max_out, int *count_host);
+
 /* Override the iteration counts of the next steps: -1 = tolerances decide, >= 0 = exactly that
  * many iterations of the divergence solve / density solve / CG.  Takes effect without re-capture.
  * Synchronises the stream. */

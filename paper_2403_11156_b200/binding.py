@@ -28,7 +28,7 @@ EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid
            "sph_read_stats", "sph_host_sync", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
            "sph_surface_workspace_bytes", "sph_surface_extract", "sph_slab_set_particles", "sph_slab_phase",
            "sph_slab_gather", "sph_slab_scatter", "sph_slab_read_error_sum", "sph_slab_set_loop", "sph_slab_store",
-           "sph_select_range", "sph_last_error", "sph_destroy"]
+           "sph_select_range", "sph_select_range_static", "sph_last_error", "sph_destroy"]
 
 
 class SphParams(C.Structure):
@@ -136,6 +136,9 @@ def load() -> C.CDLL:
         L.sph_select_range.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                        C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                                        C.c_void_p, C.c_size_t, C.POINTER(C.c_int)]
+        L.sph_select_range_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                              C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
+                                              C.POINTER(C.c_int)]
         L.sph_last_error.restype = C.c_char_p
         L.sph_last_error.argtypes = [C.c_void_p]
         L.sph_destroy.argtypes = [C.c_void_p]

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1151,6 +1152,64 @@ int sph_select_range(void *cuda_stream, const float *pos4, const float *vel4, co
     if (cudaMemcpyAsync(count_host, flag + n, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) return SPH_ECUDA;
     if (cudaStreamSynchronize(st) != cudaSuccess) return SPH_ECUDA;
     return cudaGetLastError() == cudaSuccess ? SPH_OK : SPH_ECUDA;
+}
+
+}  // extern "C"
+
+// ---- sph_select_range_static: the selection for callers that may not allocate.  Its flag / scan scratch lives in the
+// library image: one copy per GPU that loads it, held until the process exits.  In HOST code `g_select_scratch` is only
+// a stand-in for the symbol (not a device address): the per-device address comes from cudaGetSymbolAddress, looked up
+// once per device with that device current, and is what the kernels get.
+constexpr size_t kSelectStaticInts = (size_t)SPH_SELECT_STATIC_MAX + 1024;      // n + 1 flags (padded to 4) + tile sums + 4
+static __device__ __align__(256) int g_select_scratch[kSelectStaticInts];
+namespace {
+constexpr int kMaxDevices = 64;
+int *g_select_scratch_dev[kMaxDevices] = {};       // device address of g_select_scratch on device d (NULL: not looked up yet)
+std::mutex g_select_scratch_mutex;
+
+// address of the CURRENT device's copy of the array; no allocation (the array is part of the loaded module)
+int select_scratch_address(int **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { g_create_error = std::string("sph_select_range_static: cudaGetDevice failed: ") + cudaGetErrorString(e); return SPH_ECUDA; }
+    if (dev < 0 || dev >= kMaxDevices) { g_create_error = "sph_select_range_static: device ordinal beyond 63"; return SPH_EINVAL; }
+    std::lock_guard<std::mutex> lock(g_select_scratch_mutex);
+    if (!g_select_scratch_dev[dev]) {
+        int *ptr = nullptr;
+        e = cudaGetSymbolAddress((void **)&ptr, g_select_scratch);
+        if (e != cudaSuccess || !ptr) {
+            g_create_error = std::string("sph_select_range_static: cudaGetSymbolAddress failed: ") + cudaGetErrorString(e);
+            return SPH_ECUDA;
+        }
+        g_select_scratch_dev[dev] = ptr;
+    }
+    *out = g_select_scratch_dev[dev];
+    return SPH_OK;
+}
+}  // namespace
+extern "C" {
+
+int sph_select_range_static(void *cuda_stream, const float *pos4, const float *vel4, const int *gid, const int *key, int key_lt,
+                            int n, float x_lo, float x_hi, float *out_pos4, float *out_vel4, int *out_gid, int *out_idx,
+                            int max_out, int *count_host)
+{
+    if (!count_host) return SPH_EINVAL;
+    *count_host = 0;
+    if (n > SPH_SELECT_STATIC_MAX) {
+        char b[160];
+        snprintf(b, sizeof b, "sph_select_range_static: n = %d exceeds SPH_SELECT_STATIC_MAX = %d (use sph_select_range with caller scratch)",
+                 n, (int)SPH_SELECT_STATIC_MAX);
+        g_create_error = b;
+        return SPH_EINVAL;
+    }
+    int *scratch = nullptr;
+    const int rc = select_scratch_address(&scratch);
+    if (rc) return rc;
+    // the existing path, unchanged, on the library's own scratch: flag[0 .. n] and the tile sums are written by this
+    // call's first two kernels before anything reads them, so the array's stale contents never matter
+    return sph_select_range(cuda_stream, pos4, vel4, gid, key, key_lt, n, x_lo, x_hi, out_pos4, out_vel4, out_gid, out_idx,
+                            max_out, scratch, kSelectStaticInts, count_host);
 }
 
 int sph_set_forced_iterations(SphSim *s, int forced_v, int forced_d, int forced_cg)
