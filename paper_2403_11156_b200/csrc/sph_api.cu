@@ -1249,7 +1249,7 @@ int sph_read_state(SphSim *s, int field, void *dst, size_t bytes, int is_host)
         const size_t chunk = host_chunk_bytes(bytes);
         for (int k = 0; k < SphSim::kHostChunks; ++k) {
             const size_t off = (size_t)k * chunk, len = off < bytes ? (bytes - off < chunk ? bytes - off : chunk) : 0;
-            if (len > 0) CUDA_TRY(s, cudaMemcpyAsync((char *)dst + off, s->staging + off, len, cudaMemcpyDeviceToHost, s->stream));
+            if (len > 0) CUDA_TRY(s, cudaMemcpyAsync((char *)dst + off, (const char *)s->staging + off, len, cudaMemcpyDeviceToHost, s->stream));
             CUDA_TRY(s, cudaEventRecord(s->ev_chunk[k], s->stream));
         }
         s->last_read.dst = dst; s->last_read.bytes = bytes; s->last_read.seq = s->op_seq;
@@ -1282,7 +1282,7 @@ int sph_write_state(SphSim *s, int field, const void *src, size_t bytes, int is_
             for (int k = 0; k < SphSim::kHostChunks; ++k) {
                 const size_t off = (size_t)k * chunk, len = off < bytes ? (bytes - off < chunk ? bytes - off : chunk) : 0;
                 CUDA_TRY(s, cudaStreamWaitEvent(s->copy_stream, s->ev_chunk[k], 0));
-                if (len > 0) CUDA_TRY(s, cudaMemcpyAsync(s->staging_in + off, (const char *)src + off, len, cudaMemcpyHostToDevice, s->copy_stream));
+                if (len > 0) CUDA_TRY(s, cudaMemcpyAsync((char *)s->staging_in + off, (const char *)src + off, len, cudaMemcpyHostToDevice, s->copy_stream));
             }
         } else {
             CUDA_TRY(s, cudaEventRecord(s->ev_main, s->stream));
