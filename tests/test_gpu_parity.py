@@ -508,6 +508,60 @@ def test_config4_full_size_post_impact_parity(B, oracle):
     g.close(); o.close()
 
 
+def _assert_sampled_sets_by_brute_force(B, g, fp, bp, sample, h):
+    """Neighbour id sets of the sampled particles against a brute force with the fp32 predicate of reading R10 over all
+    points inside the slab |x - x_i| <= 1.01 h (a plain coordinate filter that cannot drop a neighbour; no grid)."""
+    rows_f = np_(g.sph_read_state(B.FLUID_NEIGHBORS)[torch_index(sample)])
+    rows_b = np_(g.sph_read_state(B.BOUNDARY_NEIGHBORS)[torch_index(sample)])
+    h2 = np.float32(h) * np.float32(h)
+    for r, i in enumerate(sample):
+        for pts, rows, skip in ((fp, rows_f, i), (bp, rows_b, -1)):
+            slab = np.nonzero(np.abs(pts[:, 0] - fp[i, 0]) <= np.float32(1.01 * h))[0]
+            d64 = (fp[i][None, :] - pts[slab]).astype(np.float32).astype(np.float64)
+            t = (d64[:, 0] * d64[:, 0]).astype(np.float32).astype(np.float64)
+            t = (d64[:, 1] * d64[:, 1] + t).astype(np.float32).astype(np.float64)
+            d2 = (d64[:, 2] * d64[:, 2] + t).astype(np.float32)
+            ids = set(slab[d2 < h2].tolist()) - {skip}
+            assert ids == set(int(v) for v in rows[r][rows[r] >= 0]), (i, skip)
+
+
+@pytest.mark.parametrize("n_target", [250e3, 4e6, 8e6])
+def test_sweep_sizes_sampled_and_whole_step_parity(B, oracle, n_target):
+    """The other sizes of BASELINE config 4's scaling sweep (250k, 4M and 8M fluid particles, same scene proportions), in the
+    configuration bench.py times: cell offsets and keys bit-exact and rho, alpha of EVERY particle within 1e-4 on the
+    initial state; after 100 free-running steps the neighbour sets of a seeded sample (bulk + next to walls and
+    obstacles) bit-exact against a brute force, and one resynchronised whole step (rho, alpha, v, x within 1e-4,
+    err_rho < 0.1 %)."""
+    sc = scenes.splash(n_target=n_target)
+    assert abs(sc.n_fluid - n_target) < 0.02 * n_target
+    g, o = make_pair(sc, oracle)
+    g.sph_build_grid()
+    o.build_grid(); o.compute_density_alpha()
+    st = g.sph_read_stats()
+    assert st["overflow_count"] == 0 and st["oob_count"] == 0
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_OF_PARTICLE)), o.cell_of_particle(0))
+    assert np.abs(np_(g.sph_read_state(B.DENSITY)).astype(np.float64) - o.density()).max() / 1000.0 <= TOL
+    al = o.alpha()
+    assert np.abs(np_(g.sph_read_state(B.ALPHA)).astype(np.float64) - al).max() / np.abs(al).max() <= TOL
+    g.sph_step_dfsph(100)
+    st = g.sph_read_stats()
+    assert st["steps_done"] == 100 and st["nan_count"] == 0 and st["overflow_count"] == 0 and st["oob_count"] == 0, st
+    sync_oracle_to_gpu(g, o, sc)
+    g.sph_build_grid(); o.build_grid()
+    assert np.array_equal(np_(g.sph_read_state(B.CELL_START)), o.cell_start(0))
+    cnt = np_(g.sph_read_state(B.NEIGHBOR_COUNT))
+    rng = np.random.default_rng(2)
+    near = np.nonzero(cnt[:, 1] > 0)[0]
+    sample = np.concatenate([rng.choice(g.nf, size=120, replace=False), rng.choice(near, size=80, replace=False)])
+    _assert_sampled_sets_by_brute_force(B, g, np_(g.sph_read_state(B.POS)), sc.boundary_pos, sample, sc.params["support_radius"])
+    e, st = resync_step(g, o, sc)
+    check_errors(e, sc)
+    assert st["overflow_count"] == 0 and st["nan_count"] == 0 and st["oob_count"] == 0, st
+    assert st["err_rho"] < 1e-3 and st["it_d"] >= 2
+    g.close(); o.close()
+
+
 def test_boundary_and_body_writes_take_effect(B, oracle):
     """sph_write_state of SPH_FIELD_BOUNDARY_POS / SPH_FIELD_RIGID_BODIES (include/sph.h): a static wall moved
     as a whole and a dynamic body given a new pose must reach the sorted boundary store, the Akinci volumes
