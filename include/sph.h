@@ -346,6 +346,33 @@ size_t sph_surface_workspace_bytes(const SphSurfaceParams *params);
 int sph_surface_extract(SphSim *sim, const SphSurfaceParams *params, void *workspace, size_t workspace_bytes,
                         float *triangles, long long max_triangles, long long *n_triangles);
 
+/* ---- Particle image (optional part; reading R30).  The paper renders its results with a third-party
+ * path tracer (Blender Cycles / OptiX -- unavailable here, and no equation is printed); the stand-in is
+ * an orthographic sphere splat of the fluid particles into headless DEVICE buffers, no graphics API involved:
+ *   camera   origin, orthonormal axes right / up (|right| = |up| = 1, right.up = 0 to 1e-4, else SPH_EINVAL), view direction
+ *            w = right x up; pixel (px, py), 0 <= px < width, 0 <= py < height, looks along w through
+ *            origin + (px + 1/2) pixel_size right + (py + 1/2) pixel_size up;
+ *   particle a sphere of radius `radius` (0: the simulation's particle radius) at its CURRENT position (the persistent
+ *            store: valid after sph_create, sph_write_state and every step): with (a, b, z) its camera coordinates it
+ *            covers the pixel centre (X, Y) when q = R^2 - (X - a)^2 - (Y - b)^2 > 0, at depth t = z - sqrt(q);
+ *   outputs  row-major [height][width], each may be NULL: depth = smallest t over the covering particles (+inf: empty),
+ *            id = the particle that attains it in the caller's order, the smallest id among equal depths (-1: empty),
+ *            shade = Lambert term max(0, -n.l) with the sphere normal n at the hit point and l = light / |light|, the
+ *            direction the light travels (0: empty).
+ * Deterministic: the depth / id race is decided by a 64-bit integer atomicMin.  workspace: DEVICE, 256-byte aligned,
+ * >= sph_render_workspace_bytes (8 bytes per pixel + 4 per fluid particle; 0 for invalid parameters).  Asynchronous on the
+ * simulation's stream. */
+typedef struct SphRenderParams {
+    float origin[3], right[3], up[3];
+    float pixel_size;
+    int   width, height;
+    float radius;         /* 0: particle_radius */
+    float light[3];       /* direction the light travels; not the zero vector */
+} SphRenderParams;
+size_t sph_render_workspace_bytes(const SphRenderParams *params, int n_fluid);
+int sph_render_particles(SphSim *sim, const SphRenderParams *params, void *workspace, size_t workspace_bytes,
+                         float *depth, int *id, float *shade);
+
 const char *sph_last_error(const SphSim *sim);
 void sph_destroy(SphSim *sim);
 

@@ -28,7 +28,8 @@ EXPORTS = ["sph_workspace_bytes", "sph_grid_dims", "sph_create", "sph_build_grid
            "sph_read_stats", "sph_host_sync", "sph_launch_count", "sph_enable_kernel_timing", "sph_read_kernel_times",
            "sph_surface_workspace_bytes", "sph_surface_extract", "sph_slab_set_particles", "sph_slab_phase",
            "sph_slab_gather", "sph_slab_scatter", "sph_slab_read_error_sum", "sph_slab_set_loop", "sph_slab_store",
-           "sph_select_range", "sph_select_range_static", "sph_last_error", "sph_destroy"]
+           "sph_select_range", "sph_select_range_static", "sph_render_workspace_bytes", "sph_render_particles",
+           "sph_last_error", "sph_destroy"]
 
 
 class SphParams(C.Structure):
@@ -82,6 +83,11 @@ class SphStats(C.Structure):
 
 class SphSurfaceParams(C.Structure):
     _fields_ = [("grid_min", C.c_float * 3), ("dims", C.c_int * 3), ("cube_size", C.c_float), ("iso", C.c_float)]
+
+
+class SphRenderParams(C.Structure):
+    _fields_ = [("origin", C.c_float * 3), ("right", C.c_float * 3), ("up", C.c_float * 3), ("pixel_size", C.c_float),
+                ("width", C.c_int), ("height", C.c_int), ("radius", C.c_float), ("light", C.c_float * 3)]
 
 
 class SphError(RuntimeError):
@@ -139,6 +145,10 @@ def load() -> C.CDLL:
         L.sph_select_range_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                               C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int,
                                               C.POINTER(C.c_int)]
+        L.sph_render_workspace_bytes.restype = C.c_size_t
+        L.sph_render_workspace_bytes.argtypes = [C.POINTER(SphRenderParams), C.c_int]
+        L.sph_render_particles.argtypes = [C.c_void_p, C.POINTER(SphRenderParams), C.c_void_p, C.c_size_t,
+                                           C.c_void_p, C.c_void_p, C.c_void_p]
         L.sph_last_error.restype = C.c_char_p
         L.sph_last_error.argtypes = [C.c_void_p]
         L.sph_destroy.argtypes = [C.c_void_p]
@@ -405,6 +415,32 @@ class Sim:
         nn = int(dims[0]) * int(dims[1]) * int(dims[2])
         phi = ws[off:off + 4 * nn].view(t.float32).reshape(int(dims[2]), int(dims[1]), int(dims[0]))
         return self._after_read(phi), self._after_read(tris[:min(int(n.value), max_triangles)]), int(n.value)
+
+    def sph_render_particles(self, origin, right, up, pixel_size: float, width: int, height: int, radius: float = 0.0,
+                             light=(0.0, 0.0, 1.0)):
+        """Orthographic sphere-splat image of the fluid particles (include/sph.h, reading R30).  Returns CUDA tensors
+        depth [H, W] float32 (+inf: empty), id [H, W] int32 (-1: empty), shade [H, W] float32."""
+        t = self._torch
+        rp = SphRenderParams()
+        rp.origin = (C.c_float * 3)(*[float(v) for v in origin])
+        rp.right = (C.c_float * 3)(*[float(v) for v in right])
+        rp.up = (C.c_float * 3)(*[float(v) for v in up])
+        rp.pixel_size = float(pixel_size); rp.width = int(width); rp.height = int(height); rp.radius = float(radius)
+        rp.light = (C.c_float * 3)(*[float(v) for v in light])
+        nbytes = int(load().sph_render_workspace_bytes(C.byref(rp), self.nf))
+        if nbytes == 0:
+            raise SphError(SPH_EINVAL, "sph_render_workspace_bytes rejected the camera")
+        ws = t.empty(nbytes + 256, dtype=t.uint8, device=self.device)
+        wptr = ws.data_ptr() + (-ws.data_ptr()) % 256
+        depth = t.empty((int(height), int(width)), dtype=t.float32, device=self.device)
+        pid = t.empty((int(height), int(width)), dtype=t.int32, device=self.device)
+        shade = t.empty((int(height), int(width)), dtype=t.float32, device=self.device)
+        self._stream.wait_stream(t.cuda.current_stream(self.device))
+        for x in (ws, depth, pid, shade):
+            x.record_stream(self._stream)
+        self._check(load().sph_render_particles(self._h, C.byref(rp), C.c_void_p(wptr), nbytes, C.c_void_p(depth.data_ptr()),
+                                                C.c_void_p(pid.data_ptr()), C.c_void_p(shade.data_ptr())))
+        return self._after_read(depth), self._after_read(pid), self._after_read(shade)
 
     # ---- slab mode (include/sph.h): raw device pointers in, argument marshalling only
     def sph_slab_set_particles(self, pos4, vel4, n_owned: int, n_ghost: int):

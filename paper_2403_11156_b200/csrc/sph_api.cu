@@ -16,6 +16,7 @@
 #include "sph_lists.cuh"
 #include "sph_rigid.cuh"
 #include "sph_surface.cuh"
+#include "sph_render.cuh"
 
 using namespace sph;
 
@@ -1463,6 +1464,71 @@ int sph_surface_extract(SphSim *s, const SphSurfaceParams *sp, void *workspace, 
         CUDA_TRY(s, cudaStreamSynchronize(st));
         *n_triangles = s->pinned[0];
     }
+    return SPH_OK;
+}
+
+}  // extern "C"
+namespace {
+// validates the camera and fills the kernel's view of it; false: invalid parameters
+bool render_camera(const SphRenderParams *p, float default_radius, RenderCam &c)
+{
+    if (!p || p->width < 1 || p->height < 1 || !(p->pixel_size > 0.f) || (long long)p->width * p->height > 2000000000LL) return false;
+    const double r[3] = { p->right[0], p->right[1], p->right[2] }, u[3] = { p->up[0], p->up[1], p->up[2] };
+    const double rr = r[0] * r[0] + r[1] * r[1] + r[2] * r[2], uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    const double ru = r[0] * u[0] + r[1] * u[1] + r[2] * u[2];
+    if (!(std::fabs(rr - 1.0) <= 1e-4) || !(std::fabs(uu - 1.0) <= 1e-4) || !(std::fabs(ru) <= 1e-4)) return false;
+    const double w[3] = { r[1] * u[2] - r[2] * u[1], r[2] * u[0] - r[0] * u[2], r[0] * u[1] - r[1] * u[0] };
+    const double l[3] = { p->light[0], p->light[1], p->light[2] };
+    const double ll = std::sqrt(l[0] * l[0] + l[1] * l[1] + l[2] * l[2]);
+    if (!(ll > 0.0)) return false;
+    const float R = p->radius > 0.f ? p->radius : default_radius;
+    if (!(R > 0.f) || p->radius < 0.f) return false;
+    c.ox = p->origin[0]; c.oy = p->origin[1]; c.oz = p->origin[2];
+    c.rx = (float)r[0]; c.ry = (float)r[1]; c.rz = (float)r[2];
+    c.ux = (float)u[0]; c.uy = (float)u[1]; c.uz = (float)u[2];
+    c.wx = (float)w[0]; c.wy = (float)w[1]; c.wz = (float)w[2];
+    c.lr = (float)((l[0] * r[0] + l[1] * r[1] + l[2] * r[2]) / ll);
+    c.lu = (float)((l[0] * u[0] + l[1] * u[1] + l[2] * u[2]) / ll);
+    c.lw = (float)((l[0] * w[0] + l[1] * w[1] + l[2] * w[2]) / ll);
+    c.ps = p->pixel_size; c.inv_ps = 1.0f / p->pixel_size;
+    c.R = R; c.R2 = R * R; c.inv_R = 1.0f / R;
+    c.W = p->width; c.H = p->height;
+    return true;
+}
+inline size_t render_keys_bytes(const SphRenderParams *p) { return (((size_t)p->width * (size_t)p->height * 8) + 255) & ~size_t(255); }
+}  // namespace
+extern "C" {
+
+size_t sph_render_workspace_bytes(const SphRenderParams *p, int n_fluid)
+{
+    RenderCam c;
+    if (n_fluid < 0 || !render_camera(p, 1.0f, c)) return 0;
+    return render_keys_bytes(p) + ((((size_t)(n_fluid > 0 ? n_fluid : 1) * sizeof(int)) + 255) & ~size_t(255));
+}
+
+int sph_render_particles(SphSim *s, const SphRenderParams *p, void *workspace, size_t workspace_bytes,
+                         float *depth, int *id, float *shade)
+{
+    if (!s) return SPH_EINVAL;
+    RenderCam c;
+    if (!render_camera(p, s->prm.particle_radius, c)) {
+        s->err = "render: width, height, pixel_size, radius must be positive, right / up orthonormal (1e-4), light not zero";
+        return SPH_EINVAL;
+    }
+    const size_t need = sph_render_workspace_bytes(p, s->c.nf);
+    if (!workspace || workspace_bytes < need) { s->err = "render workspace too small"; return SPH_ENOMEM; }
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0) { s->err = "render workspace must be 256-byte aligned"; return SPH_EINVAL; }
+    DeviceGuard dg(s);
+    cudaStream_t st = s->stream;
+    { int rc = join_writes(s); if (rc) return rc; }
+    unsigned long long *keys = static_cast<unsigned long long *>(workspace);
+    int *inv = reinterpret_cast<int *>(static_cast<char *>(workspace) + render_keys_bytes(p));
+    const long long npix = (long long)c.W * c.H;
+    const int nf = s->c.nf;
+    const long long nclear = npix > nf ? npix : nf;
+    LAUNCH(s, k_render_clear, cdiv(nclear, 256), 256, st, keys, npix, s->idA, nf, inv);
+    if (nf > 0) LAUNCH(s, k_render_splat, cdiv(nf, 256), 256, st, c, s->posA, s->idA, nf, keys);
+    LAUNCH(s, k_render_resolve, cdiv(npix, 256), 256, st, c, s->posA, inv, keys, depth, id, shade);
     return SPH_OK;
 }
 
