@@ -324,7 +324,7 @@ def run_ours(args):
                        "err_rho_last": st1["err_rho"], "v_max_last": st1["v_max"]},
             "clocks": ck,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nf * 24, "d2h_bytes_per_step": nf * 24,
-                    "steps": Ke, "mode": "pinned host buffers, asynchronous copies (upload of x beside download of v)"},
+                    "steps": Ke, "mode": "pinned host buffers, asynchronous copies (uploads on a second stream, chunk k of a field uploaded behind its download)"},
             "gpu_launches": int(launches),
         }
         if impact is not None:
