@@ -367,7 +367,7 @@ typedef struct SphRenderParams {
     float pixel_size;
     int   width, height;
     float radius;         /* 0: particle_radius */
-    float light[3];       /* direction the light travels; not the zero vector */
+    float light[3];       /* direction the light travels; the zero vector: the view direction w (a headlight) */
 } SphRenderParams;
 size_t sph_render_workspace_bytes(const SphRenderParams *params, int n_fluid);
 int sph_render_particles(SphSim *sim, const SphRenderParams *params, void *workspace, size_t workspace_bytes,

@@ -417,9 +417,10 @@ class Sim:
         return self._after_read(phi), self._after_read(tris[:min(int(n.value), max_triangles)]), int(n.value)
 
     def sph_render_particles(self, origin, right, up, pixel_size: float, width: int, height: int, radius: float = 0.0,
-                             light=(0.0, 0.0, 1.0)):
+                             light=(0.0, 0.0, 0.0)):
         """Orthographic sphere-splat image of the fluid particles (include/sph.h, reading R30).  Returns CUDA tensors
-        depth [H, W] float32 (+inf: empty), id [H, W] int32 (-1: empty), shade [H, W] float32."""
+        depth [H, W] float32 (+inf: empty), id [H, W] int32 (-1: empty), shade [H, W] float32.  light: the direction the
+        light travels; the zero vector (default) is a headlight along the view direction."""
         t = self._torch
         rp = SphRenderParams()
         rp.origin = (C.c_float * 3)(*[float(v) for v in origin])

@@ -1478,9 +1478,10 @@ bool render_camera(const SphRenderParams *p, float default_radius, RenderCam &c)
     const double ru = r[0] * u[0] + r[1] * u[1] + r[2] * u[2];
     if (!(std::fabs(rr - 1.0) <= 1e-4) || !(std::fabs(uu - 1.0) <= 1e-4) || !(std::fabs(ru) <= 1e-4)) return false;
     const double w[3] = { r[1] * u[2] - r[2] * u[1], r[2] * u[0] - r[0] * u[2], r[0] * u[1] - r[1] * u[0] };
-    const double l[3] = { p->light[0], p->light[1], p->light[2] };
-    const double ll = std::sqrt(l[0] * l[0] + l[1] * l[1] + l[2] * l[2]);
-    if (!(ll > 0.0)) return false;
+    double l[3] = { p->light[0], p->light[1], p->light[2] };
+    double ll = std::sqrt(l[0] * l[0] + l[1] * l[1] + l[2] * l[2]);
+    if (!(ll == ll)) return false;
+    if (ll == 0.0) { l[0] = w[0]; l[1] = w[1]; l[2] = w[2]; ll = std::sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]); }   // headlight
     const float R = p->radius > 0.f ? p->radius : default_radius;
     if (!(R > 0.f) || p->radius < 0.f) return false;
     c.ox = p->origin[0]; c.oy = p->origin[1]; c.oz = p->origin[2];
@@ -1512,7 +1513,7 @@ int sph_render_particles(SphSim *s, const SphRenderParams *p, void *workspace, s
     if (!s) return SPH_EINVAL;
     RenderCam c;
     if (!render_camera(p, s->prm.particle_radius, c)) {
-        s->err = "render: width, height, pixel_size, radius must be positive, right / up orthonormal (1e-4), light not zero";
+        s->err = "render: width, height, pixel_size must be positive, radius >= 0, right / up orthonormal (1e-4), light finite";
         return SPH_EINVAL;
     }
     const size_t need = sph_render_workspace_bytes(p, s->c.nf);

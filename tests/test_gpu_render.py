@@ -88,9 +88,13 @@ def test_render_edge_cases(B):
     # one pixel
     d, i, s = g.sph_render_particles((0, 0, -1), (1, 0, 0), (0, 1, 0), 1.0, 1, 1, radius=5.0)
     assert d.shape == (1, 1) and int(i[0, 0]) >= 0
+    # the zero light vector is a headlight: the same image as light = view direction (here right x up = +z)
+    a = g.sph_render_particles((0, 0, -1), (1, 0, 0), (0, 1, 0), 0.004, 64, 64)
+    b = g.sph_render_particles((0, 0, -1), (1, 0, 0), (0, 1, 0), 0.004, 64, 64, light=(0, 0, 2.5))
+    assert torch.equal(a[2], b[2]) and float(a[2].max()) > 0.9
     # invalid cameras / sizes are rejected, and the workspace size of an invalid camera is 0
     for kw in (dict(right=(1, 0, 0), up=(1, 0, 0)), dict(right=(2, 0, 0), up=(0, 1, 0)), dict(pixel_size=0.0),
-               dict(width=0), dict(radius=-1.0), dict(light=(0, 0, 0))):
+               dict(width=0), dict(radius=-1.0), dict(light=(float("nan"), 0, 0))):
         a = dict(origin=(0, 0, 0), right=(1, 0, 0), up=(0, 1, 0), pixel_size=0.01, width=8, height=8, radius=0.0, light=(0, 0, 1))
         a.update(kw)
         with pytest.raises(B.SphError):
